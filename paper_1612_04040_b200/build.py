@@ -1,0 +1,56 @@
+"""Build libls.so (the C-ABI library of include/ls.h) in-tree with nvcc for sm_100a.
+
+    python -m paper_1612_04040_b200.build [--force] [--verbose]
+
+nvcc cross-compiles without a GPU.  Flags that matter:
+  -gencode arch=compute_100a,code=sm_100a   B200 only, no other targets
+  -fmad=false                               no FMA contraction (arithmetic contract R18/R19)
+  -lineinfo                                 ncu source pages map to these files
+  -cudart static                            libls.so carries its own runtime; loads on a box without a driver
+"""
+from __future__ import annotations
+
+import shutil
+import subprocess
+import sys
+from pathlib import Path
+
+PKG = Path(__file__).resolve().parent
+CSRC = PKG / "csrc"
+SO = PKG / "libls.so"
+SOURCES = ["ls_band.cu", "ls_stencil.cu", "ls_api.cu"]
+NVCC_FLAGS = [
+    "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-fmad=false",
+    "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math,-Wall", "-cudart", "static", "-shared",
+]
+
+
+def nvcc_path() -> str:
+    for cand in (shutil.which("nvcc"), "/usr/local/cuda/bin/nvcc"):
+        if cand and Path(cand).exists():
+            return cand
+    raise RuntimeError("nvcc not found: libls.so cannot be built (there is no CPU fallback)")
+
+
+def needs_build() -> bool:
+    if not SO.exists():
+        return True
+    t = SO.stat().st_mtime
+    deps = [CSRC / s for s in SOURCES] + [CSRC / "ls_internal.h", PKG.parent / "include" / "ls.h", Path(__file__)]
+    return any(d.stat().st_mtime > t for d in deps)
+
+
+def build(force: bool = False, verbose: bool = False) -> Path:
+    if not force and not needs_build():
+        return SO
+    cmd = [nvcc_path(), *NVCC_FLAGS, "-o", str(SO), *[str(CSRC / s) for s in SOURCES]]
+    if verbose:
+        cmd.insert(1, "-Xptxas=-v")
+        print(" ".join(cmd), file=sys.stderr)
+    subprocess.run(cmd, check=True, cwd=str(PKG))
+    return SO
+
+
+if __name__ == "__main__":
+    build(force="--force" in sys.argv, verbose="--verbose" in sys.argv)
+    print(SO)

@@ -1,0 +1,414 @@
+// ls_api.cu — the C ABI of include/ls.h: context, argument checks, and the host driver of the
+// Step 1-3 loop on one stream.  Every step of the path runs in the kernels of
+// ls_band.cu / ls_stencil.cu; this file only sequences launches.  There is no CPU fallback.
+#include <cmath>
+#include <cstddef>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+
+#include "../../include/ls.h"
+#include "ls_internal.h"
+
+namespace ls { int scan_tile(); }
+
+struct ls_ctx {
+    ls::Geom g;
+    ls_dtype dtype;
+    cudaStream_t stream;
+    ls::BandBuffers bb;
+    void* scratch;        // one field, second Jacobi buffer (lazy)
+    void* dev_phi;        // ls_step_host staging (lazy)
+    void* dev_F;
+    unsigned long long* residual;  // device
+    ls::Counts* host_counts;       // pinned
+    unsigned long long* host_residual;  // pinned
+    bool band_valid;
+    int64_t launches;
+    int64_t dense_updates;
+    size_t elem;          // sizeof field element
+    int64_t n;            // nx*ny*nz
+};
+
+namespace {
+
+char g_cuda_error[512] = "";
+
+ls_status cuda_fail(cudaError_t e, const char* what) {
+    std::snprintf(g_cuda_error, sizeof g_cuda_error, "%s: %s", what, cudaGetErrorString(e));
+    return LS_ERR_CUDA;
+}
+
+#define LS_CK(call)                                             \
+    do {                                                        \
+        cudaError_t e_ = (call);                                \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call);     \
+    } while (0)
+
+#define LS_CK_LAUNCH()                                                   \
+    do {                                                                 \
+        cudaError_t e_ = cudaPeekAtLastError();                          \
+        if (e_ != cudaSuccess) { cudaGetLastError(); return cuda_fail(e_, "kernel launch"); } \
+    } while (0)
+
+template <typename T>
+ls::StencilParams<T> make_params(double dx, double dt, double beta, double gamma) {
+    // R18: each scalar is rounded to T once; derived constants are formed in T.
+    ls::StencilParams<T> p;
+    const T dxT = (T)dx;
+    p.inv_dx = T(1) / dxT;
+    p.dx2 = dxT * dxT;
+    p.dt = (T)dt;
+    p.beta = (T)beta;
+    p.gamma = (T)gamma;
+    p.three_beta = T(3) * p.beta;
+    const T w = p.gamma - p.beta;
+    p.inv3 = T(1) / ((w * w) * w);
+    return p;
+}
+
+ls_status ensure_field(ls_ctx* c, void** field) {
+    if (*field) return LS_OK;
+    cudaError_t e = cudaMalloc(field, (size_t)c->n * c->elem);
+    if (e != cudaSuccess) { cudaGetLastError(); *field = nullptr; return LS_ERR_ALLOC; }
+    return LS_OK;
+}
+
+bool bad_band_params(double dx, double beta, double gamma) {
+    if (!(dx > 0) || std::isnan(beta) || std::isnan(gamma)) return true;
+    if (std::isinf(beta) && std::isinf(gamma) && beta > 0 && gamma > 0) return false;
+    return !(beta > 0 && beta < gamma);
+}
+
+ls_status build_band_impl(ls_ctx* c, const void* phi, double gamma, int iters, bool count_step, bool classify) {
+    if (classify) {
+        if (c->dtype == LS_F32)
+            ls::launch_classify<float>((const float*)phi, c->g, (float)gamma, c->bb, c->stream, &c->launches);
+        else
+            ls::launch_classify<double>((const double*)phi, c->g, gamma, c->bb, c->stream, &c->launches);
+    }
+    ls::launch_dilate_compact(c->g, c->bb, iters, count_step, c->stream, &c->launches);
+    LS_CK_LAUNCH();
+    c->band_valid = true;
+    return LS_OK;
+}
+
+template <typename T>
+ls_status step_impl(ls_ctx* c, T* phi, const T* F, const ls_params* p, int n_steps) {
+    ls_status st = ensure_field(c, &c->scratch);
+    if (st != LS_OK) return st;
+    T* S = (T*)c->scratch;
+    const ls::StencilParams<T> adv = make_params<T>(p->dx, p->dt, p->beta, p->gamma);
+    const ls::StencilParams<T> rei = make_params<T>(p->dx, p->dtau, p->beta, p->gamma);
+    const T gammaT = (T)p->gamma;
+    cudaStream_t s = c->stream;
+    // Both Jacobi buffers must agree off the band: start from a full copy, and forget the previous
+    // call's N (the U list is then just N in the first step).
+    LS_CK(cudaMemcpyAsync(S, phi, (size_t)c->n * sizeof(T), cudaMemcpyDeviceToDevice, s));
+    LS_CK(cudaMemsetAsync(c->bb.flagNprev, 0, (size_t)c->g.nbricks, s));
+    bool have_T = false;  // T masks of phi^n already emitted by the previous step's last sweep
+    for (int step = 0; step < n_steps; ++step) {
+        st = build_band_impl(c, phi, p->gamma, p->iters, true, !have_T);   // Step 1
+        if (st != LS_OK) return st;
+        ls::launch_advance_band<T>(phi, F, S, c->g, adv, c->bb, false, s, &c->launches);   // Step 2: phi -> S
+        const bool emit = p->rebuild == LS_REBUILD_INCREMENTAL && step + 1 < n_steps && (p->iters & 1);
+        T* src = S;
+        T* dst = phi;
+        for (int it = 0; it < p->iters; ++it) {                             // Step 3
+            const bool last = it == p->iters - 1;
+            ls::launch_reinit_band<T>(src, dst, c->g, rei, c->bb, last, nullptr, emit && last, s, &c->launches);
+            T* t = src; src = dst; dst = t;
+        }
+        if (src != phi)  // even iters: the result sits in S
+            ls::launch_copy_clamp_band<T>(S, phi, c->g, gammaT, c->bb, s, &c->launches);
+        if (step == 0)   // eq. 10 at every point (R14); afterwards points off N already hold +-gamma
+            ls::launch_clamp_all<T>(phi, S, c->n, gammaT, s, &c->launches);
+        LS_CK_LAUNCH();
+        have_T = emit;
+        uint8_t* t = c->bb.flagN; c->bb.flagN = c->bb.flagNprev; c->bb.flagNprev = t;
+    }
+    return LS_OK;
+}
+
+ls_status check_step_args(ls_ctx* c, const void* phi, const void* F, const ls_params* p, int n_steps) {
+    if (!c || !phi || !F || !p) return LS_ERR_ARG;
+    if (n_steps < 0 || p->iters < 0) return LS_ERR_ARG;
+    if (!(p->dx > 0) || !(p->beta > 0) || !(p->beta < p->gamma) || std::isinf(p->gamma)) return LS_ERR_ARG;
+    if (p->rebuild != LS_REBUILD_FULL && p->rebuild != LS_REBUILD_INCREMENTAL) return LS_ERR_ARG;
+    return LS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* ls_status_str(ls_status s) {
+    switch (s) {
+        case LS_OK: return "LS_OK";
+        case LS_ERR_ARG: return "LS_ERR_ARG";
+        case LS_ERR_DIM: return "LS_ERR_DIM";
+        case LS_ERR_DTYPE: return "LS_ERR_DTYPE";
+        case LS_ERR_ALLOC: return "LS_ERR_ALLOC";
+        case LS_ERR_CUDA: return "LS_ERR_CUDA";
+        case LS_ERR_CAPACITY: return "LS_ERR_CAPACITY";
+        case LS_NOT_CONVERGED: return "LS_NOT_CONVERGED";
+        case LS_ERR_STATE: return "LS_ERR_STATE";
+    }
+    return "LS_UNKNOWN";
+}
+
+const char* ls_last_cuda_error(void) { return g_cuda_error; }
+
+ls_status ls_create(int32_t nx, int32_t ny, int32_t nz, ls_dtype dtype, void* cuda_stream, ls_ctx** out) {
+    if (!out) return LS_ERR_ARG;
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || nz < 1) return LS_ERR_DIM;
+    if (dtype != LS_F32 && dtype != LS_F64) return LS_ERR_DTYPE;
+    const int64_t NBx = (nx + 7) / 8, NBy = (ny + 7) / 8, NBz = (nz + 7) / 8;
+    const int64_t nbricks = NBx * NBy * NBz;
+    if (nbricks > (int64_t)1 << 27) return LS_ERR_DIM;   // brick ids, tile counts and 8*id stay in range
+    int ndev = 0;
+    LS_CK(cudaGetDeviceCount(&ndev));
+    ls_ctx* c = new (std::nothrow) ls_ctx();
+    if (!c) return LS_ERR_ALLOC;
+    std::memset(c, 0, sizeof *c);
+    c->g = ls::Geom{nx, ny, nz, (int)NBx, (int)NBy, (int)NBz, (int)nbricks};
+    c->dtype = dtype;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->elem = dtype == LS_F32 ? 4 : 8;
+    c->n = (int64_t)nx * ny * nz;
+    const int tile = ls::scan_tile();
+    const int64_t padded = (nbricks + tile - 1) / tile * tile;
+    ls::BandBuffers& bb = c->bb;
+    bb.npartials = (int)(padded / tile);
+    cudaError_t e = cudaSuccess;
+    auto alloc = [&](void** p, size_t bytes, bool zero) {
+        if (e != cudaSuccess) return;
+        e = cudaMalloc(p, bytes);
+        if (e == cudaSuccess && zero) e = cudaMemsetAsync(*p, 0, bytes, c->stream);
+    };
+    alloc((void**)&bb.tmask, (size_t)nbricks * 64, false);
+    alloc((void**)&bb.nmask, (size_t)nbricks * 64, false);
+    alloc((void**)&bb.flagT, (size_t)padded, true);
+    alloc((void**)&bb.flagN, (size_t)padded, true);
+    alloc((void**)&bb.flagNprev, (size_t)padded, true);
+    alloc((void**)&bb.T_ids, (size_t)nbricks * 4, false);
+    alloc((void**)&bb.N_ids, (size_t)nbricks * 4, false);
+    alloc((void**)&bb.U_ids, (size_t)nbricks * 4, false);
+    alloc((void**)&bb.T_masks, (size_t)nbricks * 64, false);
+    alloc((void**)&bb.N_masks, (size_t)nbricks * 64, false);
+    alloc((void**)&bb.partials, (size_t)bb.npartials * 3 * 4, true);
+    alloc((void**)&bb.counts, sizeof(ls::Counts), true);
+    alloc((void**)&c->residual, 8, true);
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&c->host_counts, sizeof(ls::Counts));
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&c->host_residual, 8);
+    if (e != cudaSuccess) {
+        const bool oom = e == cudaErrorMemoryAllocation;
+        cuda_fail(e, "ls_create allocation");
+        cudaGetLastError();
+        ls_destroy(c);
+        return oom ? LS_ERR_ALLOC : LS_ERR_CUDA;
+    }
+    *out = c;
+    return LS_OK;
+}
+
+ls_status ls_destroy(ls_ctx* c) {
+    if (!c) return LS_OK;
+    cudaStreamSynchronize(c->stream);
+    ls::BandBuffers& bb = c->bb;
+    void* dev[] = {bb.tmask, bb.nmask, bb.flagT, bb.flagN, bb.flagNprev, bb.T_ids, bb.N_ids, bb.U_ids,
+                   bb.T_masks, bb.N_masks, bb.partials, bb.counts, c->residual, c->scratch, c->dev_phi, c->dev_F};
+    for (void* p : dev)
+        if (p) cudaFree(p);
+    if (c->host_counts) cudaFreeHost(c->host_counts);
+    if (c->host_residual) cudaFreeHost(c->host_residual);
+    cudaGetLastError();
+    delete c;
+    return LS_OK;
+}
+
+ls_status ls_build_band(ls_ctx* c, const void* phi, double dx, double gamma) {
+    if (!c || !phi) return LS_ERR_ARG;
+    if (!(dx > 0) || !(gamma > 0)) return LS_ERR_ARG;
+    LS_CK(cudaMemsetAsync(c->bb.flagNprev, 0, (size_t)c->g.nbricks, c->stream));
+    return build_band_impl(c, phi, gamma, 0, false, true);
+}
+
+ls_status ls_band_counts(ls_ctx* c, int64_t* nT_points, int64_t* nN_points, int32_t* nT_bricks, int32_t* nN_bricks) {
+    if (!c) return LS_ERR_ARG;
+    if (!c->band_valid) return LS_ERR_STATE;
+    LS_CK(cudaMemcpyAsync(c->host_counts, c->bb.counts, sizeof(ls::Counts), cudaMemcpyDeviceToHost, c->stream));
+    LS_CK(cudaStreamSynchronize(c->stream));
+    if (nT_points) *nT_points = (int64_t)c->host_counts->nT_pts;
+    if (nN_points) *nN_points = (int64_t)c->host_counts->nN_pts;
+    if (nT_bricks) *nT_bricks = c->host_counts->nT;
+    if (nN_bricks) *nN_bricks = c->host_counts->nN;
+    return LS_OK;
+}
+
+ls_status ls_band_export(ls_ctx* c, int32_t* T_ids, uint64_t* T_masks, int32_t* N_ids, uint64_t* N_masks) {
+    int32_t nT = 0, nN = 0;
+    ls_status st = ls_band_counts(c, nullptr, nullptr, &nT, &nN);
+    if (st != LS_OK) return st;
+    cudaStream_t s = c->stream;
+    if (T_ids && nT) LS_CK(cudaMemcpyAsync(T_ids, c->bb.T_ids, (size_t)nT * 4, cudaMemcpyDeviceToHost, s));
+    if (T_masks && nT) LS_CK(cudaMemcpyAsync(T_masks, c->bb.T_masks, (size_t)nT * 64, cudaMemcpyDeviceToHost, s));
+    if (N_ids && nN) LS_CK(cudaMemcpyAsync(N_ids, c->bb.N_ids, (size_t)nN * 4, cudaMemcpyDeviceToHost, s));
+    if (N_masks && nN) LS_CK(cudaMemcpyAsync(N_masks, c->bb.N_masks, (size_t)nN * 64, cudaMemcpyDeviceToHost, s));
+    LS_CK(cudaStreamSynchronize(s));
+    return LS_OK;
+}
+
+ls_status ls_advance(ls_ctx* c, const void* phi, const void* F, double dt, double dx, double beta, double gamma,
+                     void* out) {
+    if (!c || !phi || !F || !out || out == phi) return LS_ERR_ARG;
+    if (bad_band_params(dx, beta, gamma)) return LS_ERR_ARG;
+    const bool dense = std::isinf(beta) && std::isinf(gamma);
+    cudaStream_t s = c->stream;
+    if (dense) {
+        if (c->dtype == LS_F32)
+            ls::launch_advance_dense<float>((const float*)phi, (const float*)F, (float*)out, c->g,
+                                            make_params<float>(dx, dt, beta, gamma), s, &c->launches);
+        else
+            ls::launch_advance_dense<double>((const double*)phi, (const double*)F, (double*)out, c->g,
+                                             make_params<double>(dx, dt, beta, gamma), s, &c->launches);
+        LS_CK_LAUNCH();
+        c->dense_updates += c->n;
+        return LS_OK;
+    }
+    if (!c->band_valid) return LS_ERR_STATE;
+    // out = phi everywhere, then eq. 8 on the T bricks.
+    LS_CK(cudaMemcpyAsync(out, phi, (size_t)c->n * c->elem, cudaMemcpyDeviceToDevice, s));
+    if (c->dtype == LS_F32)
+        ls::launch_advance_band<float>((const float*)phi, (const float*)F, (float*)out, c->g,
+                                       make_params<float>(dx, dt, beta, gamma), c->bb, true, s, &c->launches);
+    else
+        ls::launch_advance_band<double>((const double*)phi, (const double*)F, (double*)out, c->g,
+                                        make_params<double>(dx, dt, beta, gamma), c->bb, true, s, &c->launches);
+    LS_CK_LAUNCH();
+    return LS_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+// Shared body of ls_reinit (tol < 0: fixed count) and ls_reinit_tol.
+template <typename T>
+ls_status reinit_impl(ls_ctx* c, T* d, const T* phi_bar, double dtau, double dx, double gamma, int iters, double tol,
+                      int check_every, int32_t* iters_done, double* residual_out) {
+    ls_status st = ensure_field(c, &c->scratch);
+    if (st != LS_OK) return st;
+    T* S = (T*)c->scratch;
+    cudaStream_t s = c->stream;
+    const size_t bytes = (size_t)c->n * sizeof(T);
+    const ls::StencilParams<T> rei = make_params<T>(dx, dtau, gamma * 0.5, gamma);
+    LS_CK(cudaMemcpyAsync(d, phi_bar, bytes, cudaMemcpyDeviceToDevice, s));
+    LS_CK(cudaMemcpyAsync(S, phi_bar, bytes, cudaMemcpyDeviceToDevice, s));
+    const bool to_tol = tol >= 0;
+    // fixed count: choose the first source so that the last sweep writes d
+    T* src = (!to_tol && (iters & 1)) ? S : d;
+    T* dst = src == d ? S : d;
+    int k = 0;
+    double r = 0.0;
+    bool converged = false;
+    while (k < iters) {
+        ++k;
+        const bool check = to_tol && (k % check_every == 0 || k == iters);
+        if (check) LS_CK(cudaMemsetAsync(c->residual, 0, 8, s));
+        ls::launch_reinit_band<T>(src, dst, c->g, rei, c->bb, false, check ? c->residual : nullptr, false, s,
+                                  &c->launches);
+        T* t = src; src = dst; dst = t;
+        if (check) {
+            LS_CK_LAUNCH();
+            LS_CK(cudaMemcpyAsync(c->host_residual, c->residual, 8, cudaMemcpyDeviceToHost, s));
+            LS_CK(cudaStreamSynchronize(s));
+            const unsigned long long bits = *c->host_residual;
+            if (sizeof(T) == 4) { uint32_t b32 = (uint32_t)bits; float f; std::memcpy(&f, &b32, 4); r = f; }
+            else std::memcpy(&r, &bits, 8);
+            if (k % check_every == 0 && r < tol) { converged = true; break; }
+        }
+    }
+    LS_CK_LAUNCH();
+    if (src != d) LS_CK(cudaMemcpyAsync(d, src, bytes, cudaMemcpyDeviceToDevice, s));   // result is in `src`
+    ls::launch_clamp_all<T>(d, (T*)nullptr, c->n, (T)gamma, s, &c->launches);          // eq. 10 everywhere
+    LS_CK_LAUNCH();
+    if (iters_done) *iters_done = k;
+    if (residual_out) *residual_out = r;
+    if (to_tol && !converged) return LS_NOT_CONVERGED;
+    return LS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+ls_status ls_reinit(ls_ctx* c, void* d, const void* phi_bar, double dtau, double dx, double gamma, int32_t iters) {
+    if (!c || !d || !phi_bar || d == phi_bar) return LS_ERR_ARG;
+    if (!(dx > 0) || !(gamma > 0) || std::isinf(gamma) || iters < 0) return LS_ERR_ARG;
+    if (!c->band_valid) return LS_ERR_STATE;
+    if (c->dtype == LS_F32)
+        return reinit_impl<float>(c, (float*)d, (const float*)phi_bar, dtau, dx, gamma, iters, -1.0, 1, nullptr, nullptr);
+    return reinit_impl<double>(c, (double*)d, (const double*)phi_bar, dtau, dx, gamma, iters, -1.0, 1, nullptr, nullptr);
+}
+
+ls_status ls_reinit_tol(ls_ctx* c, void* d, const void* phi_bar, double dtau, double dx, double gamma, double tol,
+                        int32_t max_iters, int32_t check_every, int32_t* iters_done, double* residual) {
+    if (!c || !d || !phi_bar || d == phi_bar) return LS_ERR_ARG;
+    if (!(dx > 0) || !(gamma > 0) || std::isinf(gamma) || max_iters < 0 || check_every < 1 || !(tol >= 0))
+        return LS_ERR_ARG;
+    if (!c->band_valid) return LS_ERR_STATE;
+    if (c->dtype == LS_F32)
+        return reinit_impl<float>(c, (float*)d, (const float*)phi_bar, dtau, dx, gamma, max_iters, tol, check_every,
+                                  iters_done, residual);
+    return reinit_impl<double>(c, (double*)d, (const double*)phi_bar, dtau, dx, gamma, max_iters, tol, check_every,
+                               iters_done, residual);
+}
+
+ls_status ls_step(ls_ctx* c, void* phi, const void* F, const ls_params* p, int32_t n_steps) {
+    ls_status st = check_step_args(c, phi, F, p, n_steps);
+    if (st != LS_OK) return st;
+    if (n_steps == 0) return LS_OK;
+    if (c->dtype == LS_F32) return step_impl<float>(c, (float*)phi, (const float*)F, p, n_steps);
+    return step_impl<double>(c, (double*)phi, (const double*)F, p, n_steps);
+}
+
+ls_status ls_step_host(ls_ctx* c, void* phi_host, const void* F_host, const ls_params* p, int32_t n_steps) {
+    ls_status st = check_step_args(c, phi_host, F_host, p, n_steps);
+    if (st != LS_OK) return st;
+    if ((st = ensure_field(c, &c->dev_phi)) != LS_OK) return st;
+    if ((st = ensure_field(c, &c->dev_F)) != LS_OK) return st;
+    const size_t bytes = (size_t)c->n * c->elem;
+    LS_CK(cudaMemcpyAsync(c->dev_phi, phi_host, bytes, cudaMemcpyHostToDevice, c->stream));
+    LS_CK(cudaMemcpyAsync(c->dev_F, F_host, bytes, cudaMemcpyHostToDevice, c->stream));
+    if (n_steps > 0) {
+        st = c->dtype == LS_F32 ? step_impl<float>(c, (float*)c->dev_phi, (const float*)c->dev_F, p, n_steps)
+                                : step_impl<double>(c, (double*)c->dev_phi, (const double*)c->dev_F, p, n_steps);
+        if (st != LS_OK) return st;
+    }
+    LS_CK(cudaMemcpyAsync(phi_host, c->dev_phi, bytes, cudaMemcpyDeviceToHost, c->stream));
+    LS_CK(cudaStreamSynchronize(c->stream));
+    return LS_OK;
+}
+
+ls_status ls_stats(ls_ctx* c, int64_t* point_updates, int64_t* steps, int64_t* kernel_launches) {
+    if (!c) return LS_ERR_ARG;
+    LS_CK(cudaMemcpyAsync(c->host_counts, c->bb.counts, sizeof(ls::Counts), cudaMemcpyDeviceToHost, c->stream));
+    LS_CK(cudaStreamSynchronize(c->stream));
+    if (point_updates) *point_updates = (int64_t)c->host_counts->updates + c->dense_updates;
+    if (steps) *steps = (int64_t)c->host_counts->steps;
+    if (kernel_launches) *kernel_launches = c->launches;
+    return LS_OK;
+}
+
+ls_status ls_stats_reset(ls_ctx* c) {
+    if (!c) return LS_ERR_ARG;
+    LS_CK(cudaMemsetAsync((char*)c->bb.counts + offsetof(ls::Counts, updates), 0, 16, c->stream));
+    c->launches = 0;
+    c->dense_updates = 0;
+    return LS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,382 @@
+// ls_stencil.cu — Steps 2 and 3: the first-order upwind update of eq. 3-5
+// with the cut-off of eq. 7/8, the reinitialisation sweep of
+// eq. 12-13 and the clamp of eq. 10.
+//
+// Arithmetic contract (R18, R19): everything in T, IEEE divide / square root, no FMA contraction
+// (this file is compiled with -fmad=false), differences scaled by inv_dx = 1/dx, the six squared
+// terms summed pairwise by axis ((x-pair + y-pair) + z-pair).  Only the gradient norm that the sign
+// of F (or of d) selects is rooted: the other one is multiplied by an exact zero in eq. 3.
+#include "ls_internal.h"
+
+namespace ls {
+
+namespace {
+
+constexpr int kBandThreads = 256;
+constexpr int kTileEdge = 10;                 // 8 + one halo cell on each side
+constexpr int kTileElems = kTileEdge * kTileEdge * kTileEdge;
+
+template <typename T> __device__ __forceinline__ T pos(T x) { return x > T(0) ? x : T(0); }   // max(x, 0)
+template <typename T> __device__ __forceinline__ T neg(T x) { return x < T(0) ? x : T(0); }   // min(x, 0)
+template <typename T> __device__ __forceinline__ T root(T x);
+template <> __device__ __forceinline__ float root<float>(float x) { return __fsqrt_rn(x); }
+template <> __device__ __forceinline__ double root<double>(double x) { return __dsqrt_rn(x); }
+template <typename T> __device__ __forceinline__ T quot(T a, T b);
+template <> __device__ __forceinline__ float quot<float>(float a, float b) { return __fdiv_rn(a, b); }
+template <> __device__ __forceinline__ double quot<double>(double a, double b) { return __ddiv_rn(a, b); }
+template <typename T> __device__ __forceinline__ T mag(T v);
+template <> __device__ __forceinline__ float mag<float>(float v) { return fabsf(v); }
+template <> __device__ __forceinline__ double mag<double>(double v) { return fabs(v); }
+
+// q+ = (grad+)^2 of eq. 4 and q- = (grad-)^2 of eq. 5 from the 7-point star.
+template <typename T>
+__device__ __forceinline__ void upwind_q(T c, T xm, T xp, T ym, T yp, T zm, T zp, T inv, T& qp, T& qm) {
+    const T Dmx = (c - xm) * inv, Dpx = (xp - c) * inv;
+    const T Dmy = (c - ym) * inv, Dpy = (yp - c) * inv;
+    const T Dmz = (c - zm) * inv, Dpz = (zp - c) * inv;
+    const T amx = pos(Dmx), bmx = neg(Dmx), apx = pos(Dpx), bpx = neg(Dpx);
+    const T amy = pos(Dmy), bmy = neg(Dmy), apy = pos(Dpy), bpy = neg(Dpy);
+    const T amz = pos(Dmz), bmz = neg(Dmz), apz = pos(Dpz), bpz = neg(Dpz);
+    qp = ((amx * amx + bpx * bpx) + (amy * amy + bpy * bpy)) + (amz * amz + bpz * bpz);
+    qm = ((apx * apx + bmx * bmx) + (apy * apy + bmy * bmy)) + (apz * apz + bmz * bmz);
+}
+
+// eq. 7 (R5: test <= beta, then <= gamma, else 0)
+template <typename T>
+__device__ __forceinline__ T cutoff(T c, const StencilParams<T>& p) {
+    const T a = mag(c);
+    if (a <= p.beta) return T(1);
+    if (a <= p.gamma) {
+        const T t = a - p.gamma;
+        return ((t * t) * (((T(2) * a) + p.gamma) - p.three_beta)) * p.inv3;
+    }
+    return T(0);
+}
+
+// eq. 3 with eq. 8: phi - dt * (c(phi) * [max(F,0) grad+ + min(F,0) grad-]).
+template <typename T, bool DENSE>
+__device__ __forceinline__ T advance_value(T c, T xm, T xp, T ym, T yp, T zm, T zp, T f, const StencilParams<T>& p) {
+    T qp, qm;
+    upwind_q(c, xm, xp, ym, yp, zm, zp, p.inv_dx, qp, qm);
+    // f > 0: H = f*grad+ + 0*grad-;  f < 0: H = 0*grad+ + f*grad-;  f == 0: H = 0
+    const T H = f * root(f > T(0) ? qp : qm);
+    const T cf = DENSE ? T(1) : cutoff(c, p);
+    return c - p.dt * (cf * H);
+}
+
+// eq. 12-13 (R9-R12): d - dtau * [max(S,0)(grad+ - 1) + min(S,0)(grad- - 1)], S = d / sqrt(d^2 + |Dd|^2 dx^2),
+// |Dd|^2 = q+ if d > 0, q- if d < 0; S = 0 where the root vanishes.
+template <typename T>
+__device__ __forceinline__ T reinit_value(T c, T xm, T xp, T ym, T yp, T zm, T zp, const StencilParams<T>& p) {
+    T qp, qm;
+    upwind_q(c, xm, xp, ym, yp, zm, zp, p.inv_dx, qp, qm);
+    const T q = c > T(0) ? qp : (c < T(0) ? qm : T(0));
+    const T den = root(c * c + q * p.dx2);
+    const T S = den == T(0) ? T(0) : quot(c, den);
+    const T U = S * (root(q) - T(1));   // sign S = sign d picks the branch; the other term is an exact 0
+    return c - p.dt * U;
+}
+
+template <typename T>
+__device__ __forceinline__ T clamp_val(T v, T gamma) {
+    if (v < -gamma) v = -gamma;
+    if (v > gamma) v = gamma;
+    return v;
+}
+
+// Stage brick (x0,y0,z0) plus its six faces into s[z][y][x] (10^3, edges/corners skipped).
+// Indices are clamped to the domain: edge replicate (R3).
+template <typename T>
+__device__ __forceinline__ void load_halo_tile(T* __restrict__ s, const T* __restrict__ src, const Geom& g, int x0,
+                                               int y0, int z0) {
+    for (int e = threadIdx.x; e < kTileElems; e += kBandThreads) {
+        const int x = e % kTileEdge, r = e / kTileEdge;
+        const int y = r % kTileEdge, z = r / kTileEdge;
+        const int on_face = (x == 0 || x == kTileEdge - 1) + (y == 0 || y == kTileEdge - 1) +
+                            (z == 0 || z == kTileEdge - 1);
+        if (on_face > 1) continue;
+        const int i = min(max(x0 + x - 1, 0), g.nx - 1);
+        const int j = min(max(y0 + y - 1, 0), g.ny - 1);
+        const int k = min(max(z0 + z - 1, 0), g.nz - 1);
+        s[e] = __ldg(src + g.idx(i, j, k));
+    }
+}
+
+#define LS_TILE(s, lx, ly, lz) (s)[(((lz) + 1) * kTileEdge + ((ly) + 1)) * kTileEdge + ((lx) + 1)]
+
+// Advance over a brick list.  Writes every in-domain point of each listed brick.
+template <typename T>
+__global__ void __launch_bounds__(kBandThreads) k_advance_band(const T* __restrict__ phi, const T* __restrict__ F,
+                                                               T* __restrict__ out, Geom g, StencilParams<T> p,
+                                                               const int32_t* __restrict__ ids,
+                                                               const int32_t* __restrict__ count_ptr,
+                                                               const uint64_t* __restrict__ list_masks,
+                                                               const uint64_t* __restrict__ tmask,
+                                                               const uint8_t* __restrict__ flagT) {
+    __shared__ T s[kTileElems];
+    const int count = *count_ptr;
+    const int lx = threadIdx.x & 7, ly = (threadIdx.x >> 3) & 7, lz0 = threadIdx.x >> 6;
+    for (int li = blockIdx.x; li < count; li += gridDim.x) {
+        const int b = ids[li];
+        const int bx = b % g.NBx, by = (b / g.NBx) % g.NBy, bz = b / (g.NBx * g.NBy);
+        const int x0 = bx * 8, y0 = by * 8, z0 = bz * 8;
+        load_halo_tile(s, phi, g, x0, y0, z0);
+        const bool has_T = list_masks ? true : (flagT[b] != 0);
+        __syncthreads();
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int lz = lz0 + 4 * h;
+            const int i = x0 + lx, j = y0 + ly, k = z0 + lz;
+            if (i < g.nx && j < g.ny && k < g.nz) {
+                uint64_t w = 0;
+                if (has_T) w = list_masks ? list_masks[(int64_t)li * 8 + lz] : tmask[(int64_t)b * 8 + lz];
+                const T c = LS_TILE(s, lx, ly, lz);
+                T v = c;
+                const int64_t at = g.idx(i, j, k);
+                if ((w >> (ly * 8 + lx)) & 1ull) {
+                    v = advance_value<T, false>(c, LS_TILE(s, lx - 1, ly, lz), LS_TILE(s, lx + 1, ly, lz),
+                                                LS_TILE(s, lx, ly - 1, lz), LS_TILE(s, lx, ly + 1, lz),
+                                                LS_TILE(s, lx, ly, lz - 1), LS_TILE(s, lx, ly, lz + 1), __ldg(F + at), p);
+                }
+                out[at] = v;
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// One reinit sweep over the N list (see launch_reinit_band in ls_internal.h).
+template <typename T, bool CLAMP, bool RESIDUAL, bool EMIT_T>
+__global__ void __launch_bounds__(kBandThreads) k_reinit_band(const T* __restrict__ src, T* __restrict__ dst, Geom g,
+                                                              StencilParams<T> p, const int32_t* __restrict__ ids,
+                                                              const int32_t* __restrict__ count_ptr,
+                                                              const uint64_t* __restrict__ masks,
+                                                              unsigned long long* __restrict__ residual,
+                                                              uint64_t* __restrict__ tmask, uint8_t* __restrict__ flagT) {
+    __shared__ T s[kTileElems];
+    __shared__ uint32_t halves[8][2];
+    const int count = *count_ptr;
+    const int lx = threadIdx.x & 7, ly = (threadIdx.x >> 3) & 7, lz0 = threadIdx.x >> 6;
+    T rmax = T(0);
+    for (int li = blockIdx.x; li < count; li += gridDim.x) {
+        const int b = ids[li];
+        const int bx = b % g.NBx, by = (b / g.NBx) % g.NBy, bz = b / (g.NBx * g.NBy);
+        const int x0 = bx * 8, y0 = by * 8, z0 = bz * 8;
+        load_halo_tile(s, src, g, x0, y0, z0);
+        __syncthreads();
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int lz = lz0 + 4 * h;
+            const int i = x0 + lx, j = y0 + ly, k = z0 + lz;
+            const uint64_t w = masks[(int64_t)li * 8 + lz];
+            const unsigned rowbits = (unsigned)(w >> (ly * 8)) & 0xffu;
+            const bool active = (rowbits >> lx) & 1u;
+            bool tbit = false;
+            if (rowbits != 0 && i < g.nx && j < g.ny && k < g.nz) {
+                const T c = LS_TILE(s, lx, ly, lz);
+                T v = c;
+                if (active) {
+                    v = reinit_value<T>(c, LS_TILE(s, lx - 1, ly, lz), LS_TILE(s, lx + 1, ly, lz),
+                                        LS_TILE(s, lx, ly - 1, lz), LS_TILE(s, lx, ly + 1, lz),
+                                        LS_TILE(s, lx, ly, lz - 1), LS_TILE(s, lx, ly, lz + 1), p);
+                    if (RESIDUAL) rmax = fmax(rmax, mag(v - c));
+                }
+                if (CLAMP) v = clamp_val(v, p.gamma);
+                if (EMIT_T) tbit = active && mag(v) < p.gamma;
+                dst[g.idx(i, j, k)] = v;
+            }
+            if (EMIT_T) {
+                // this warp holds rows 4*(warp&1) .. +3 of layer lz: lane == bit index within the half word
+                const unsigned hw = __ballot_sync(0xffffffffu, tbit);
+                if ((threadIdx.x & 31) == 0) halves[lz][(threadIdx.x >> 5) & 1] = hw;
+            }
+        }
+        __syncthreads();
+        if (EMIT_T && threadIdx.x < 32) {
+            uint64_t word = 0;
+            if (threadIdx.x < 8) word = (uint64_t)halves[threadIdx.x][0] | ((uint64_t)halves[threadIdx.x][1] << 32);
+            const bool any = __ballot_sync(0xffffffffu, word != 0) != 0;
+            if (threadIdx.x < 8 && any) tmask[(int64_t)b * 8 + threadIdx.x] = word;
+            if (threadIdx.x == 0) flagT[b] = any ? 1 : 0;
+        }
+        if (EMIT_T) __syncthreads();
+    }
+    if (RESIDUAL) {
+        // non-negative IEEE values order like their bit patterns
+        unsigned long long bits;
+        if (sizeof(T) == 4) bits = (unsigned long long)__float_as_uint((float)rmax);
+        else bits = (unsigned long long)__double_as_longlong((double)rmax);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const unsigned long long y = __shfl_xor_sync(0xffffffffu, bits, o);
+            bits = y > bits ? y : bits;
+        }
+        if ((threadIdx.x & 31) == 0 && bits != 0) atomicMax(residual, bits);
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kBandThreads) k_copy_clamp_band(const T* __restrict__ src, T* __restrict__ dst, Geom g,
+                                                                  T gamma, const int32_t* __restrict__ ids,
+                                                                  const int32_t* __restrict__ count_ptr,
+                                                                  const uint64_t* __restrict__ masks) {
+    const int count = *count_ptr;
+    const int lx = threadIdx.x & 7, ly = (threadIdx.x >> 3) & 7, lz0 = threadIdx.x >> 6;
+    for (int li = blockIdx.x; li < count; li += gridDim.x) {
+        const int b = ids[li];
+        const int bx = b % g.NBx, by = (b / g.NBx) % g.NBy, bz = b / (g.NBx * g.NBy);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int lz = lz0 + 4 * h;
+            const int i = bx * 8 + lx, j = by * 8 + ly, k = bz * 8 + lz;
+            const uint64_t w = masks[(int64_t)li * 8 + lz];
+            if (((w >> (ly * 8)) & 0xffull) != 0 && i < g.nx && j < g.ny && k < g.nz) {
+                const int64_t at = g.idx(i, j, k);
+                dst[at] = clamp_val(src[at], gamma);
+            }
+        }
+    }
+}
+
+// Full-domain advance, c == 1 (cfg 2).  CTA = 32(x) x 8(y) columns marching over a z chunk; the
+// z-neighbours rotate through registers, x/y neighbours come through L1.
+constexpr int kDenseZ = 16;
+template <typename T>
+__global__ void __launch_bounds__(256) k_advance_dense(const T* __restrict__ phi, const T* __restrict__ F,
+                                                       T* __restrict__ out, Geom g, StencilParams<T> p) {
+    const int i = blockIdx.x * 32 + threadIdx.x;
+    const int j = blockIdx.y * 8 + threadIdx.y;
+    const int k0 = blockIdx.z * kDenseZ;
+    if (i >= g.nx || j >= g.ny) return;
+    const int im = max(i - 1, 0), ip = min(i + 1, g.nx - 1);
+    const int jm = max(j - 1, 0), jp = min(j + 1, g.ny - 1);
+    const int k1 = min(k0 + kDenseZ, g.nz);
+    T zm = __ldg(phi + g.idx(i, j, max(k0 - 1, 0)));
+    T c = __ldg(phi + g.idx(i, j, k0));
+    for (int k = k0; k < k1; ++k) {
+        const T zp = __ldg(phi + g.idx(i, j, min(k + 1, g.nz - 1)));
+        const T xm = __ldg(phi + g.idx(im, j, k)), xp = __ldg(phi + g.idx(ip, j, k));
+        const T ym = __ldg(phi + g.idx(i, jm, k)), yp = __ldg(phi + g.idx(i, jp, k));
+        const int64_t at = g.idx(i, j, k);
+        out[at] = advance_value<T, true>(c, xm, xp, ym, yp, zm, zp, __ldg(F + at), p);
+        zm = c;
+        c = zp;
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_clamp_all(T* __restrict__ a, T* __restrict__ b, int64_t n, T gamma) {
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += stride) {
+        const T v = a[p];
+        const T c = clamp_val(v, gamma);
+        if (c != v) {
+            a[p] = c;
+            if (b) b[p] = c;
+        }
+    }
+}
+
+// 128-bit variant for fp32 fields whose size is a multiple of 4.
+__global__ void __launch_bounds__(256) k_clamp_all_v4(float4* __restrict__ a, float4* __restrict__ b, int64_t n4,
+                                                      float gamma) {
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n4; p += stride) {
+        const float4 v = a[p];
+        float4 c;
+        c.x = clamp_val(v.x, gamma); c.y = clamp_val(v.y, gamma);
+        c.z = clamp_val(v.z, gamma); c.w = clamp_val(v.w, gamma);
+        if (c.x != v.x || c.y != v.y || c.z != v.z || c.w != v.w) {
+            a[p] = c;
+            if (b) b[p] = c;
+        }
+    }
+}
+
+int band_grid() { return sm_count() * 8; }
+
+}  // namespace
+
+int sm_count() {
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0)
+            n = 148;
+    }
+    return n;
+}
+
+template <typename T>
+void launch_advance_band(const T* phi, const T* F, T* out, const Geom& g, const StencilParams<T>& p,
+                         const BandBuffers& bb, bool use_T_list, cudaStream_t s, int64_t* launches) {
+    if (use_T_list)
+        k_advance_band<T><<<band_grid(), kBandThreads, 0, s>>>(phi, F, out, g, p, bb.T_ids, &bb.counts->nT, bb.T_masks,
+                                                               nullptr, nullptr);
+    else
+        k_advance_band<T><<<band_grid(), kBandThreads, 0, s>>>(phi, F, out, g, p, bb.U_ids, &bb.counts->nU, nullptr,
+                                                               bb.tmask, bb.flagT);
+    if (launches) *launches += 1;
+}
+
+template <typename T>
+void launch_advance_dense(const T* phi, const T* F, T* out, const Geom& g, const StencilParams<T>& p, cudaStream_t s,
+                          int64_t* launches) {
+    dim3 block(32, 8, 1);
+    dim3 grid((g.nx + 31) / 32, (g.ny + 7) / 8, (g.nz + kDenseZ - 1) / kDenseZ);
+    k_advance_dense<T><<<grid, block, 0, s>>>(phi, F, out, g, p);
+    if (launches) *launches += 1;
+}
+
+template <typename T>
+void launch_reinit_band(const T* src, T* dst, const Geom& g, const StencilParams<T>& p, const BandBuffers& bb,
+                        bool clamp, unsigned long long* residual, bool emit_T, cudaStream_t s, int64_t* launches) {
+    const int grid = band_grid();
+    const int32_t* cnt = &bb.counts->nN;
+#define LS_LAUNCH(C, R, E)                                                                                        \
+    k_reinit_band<T, C, R, E><<<grid, kBandThreads, 0, s>>>(src, dst, g, p, bb.N_ids, cnt, bb.N_masks, residual, \
+                                                            bb.tmask, bb.flagT)
+    if (emit_T) LS_LAUNCH(true, false, true);
+    else if (residual && clamp) LS_LAUNCH(true, true, false);
+    else if (residual) LS_LAUNCH(false, true, false);
+    else if (clamp) LS_LAUNCH(true, false, false);
+    else LS_LAUNCH(false, false, false);
+#undef LS_LAUNCH
+    if (launches) *launches += 1;
+}
+
+template <typename T>
+void launch_copy_clamp_band(const T* src, T* dst, const Geom& g, T gamma, const BandBuffers& bb, cudaStream_t s,
+                            int64_t* launches) {
+    k_copy_clamp_band<T><<<band_grid(), kBandThreads, 0, s>>>(src, dst, g, gamma, bb.N_ids, &bb.counts->nN, bb.N_masks);
+    if (launches) *launches += 1;
+}
+
+template <typename T>
+void launch_clamp_all(T* a, T* b, int64_t n, T gamma, cudaStream_t s, int64_t* launches) {
+    const int grid = sm_count() * 16;
+    if (sizeof(T) == 4 && n % 4 == 0 && (reinterpret_cast<uintptr_t>(a) & 15) == 0 &&
+        (reinterpret_cast<uintptr_t>(b) & 15) == 0) {
+        k_clamp_all_v4<<<grid, 256, 0, s>>>(reinterpret_cast<float4*>(a), reinterpret_cast<float4*>(b), n / 4,
+                                            (float)gamma);
+    } else {
+        k_clamp_all<T><<<grid, 256, 0, s>>>(a, b, n, gamma);
+    }
+    if (launches) *launches += 1;
+}
+
+#define LS_INSTANTIATE(T)                                                                                          \
+    template void launch_advance_band<T>(const T*, const T*, T*, const Geom&, const StencilParams<T>&,            \
+                                         const BandBuffers&, bool, cudaStream_t, int64_t*);                        \
+    template void launch_advance_dense<T>(const T*, const T*, T*, const Geom&, const StencilParams<T>&,           \
+                                          cudaStream_t, int64_t*);                                                 \
+    template void launch_reinit_band<T>(const T*, T*, const Geom&, const StencilParams<T>&, const BandBuffers&,   \
+                                        bool, unsigned long long*, bool, cudaStream_t, int64_t*);                  \
+    template void launch_copy_clamp_band<T>(const T*, T*, const Geom&, T, const BandBuffers&, cudaStream_t,       \
+                                            int64_t*);                                                             \
+    template void launch_clamp_all<T>(T*, T*, int64_t, T, cudaStream_t, int64_t*);
+LS_INSTANTIATE(float)
+LS_INSTANTIATE(double)
+
+}  // namespace ls

@@ -1,0 +1,81 @@
+"""CPU-side checks of the boundary: libls.so builds, loads without a GPU, exports every symbol that
+include/ls.h declares, rejects bad arguments before touching CUDA, and fails loudly (no fallback)
+when there is no device."""
+import ctypes as C
+import re
+from pathlib import Path
+
+import pytest
+
+from paper_1612_04040_b200 import binding as ls
+from paper_1612_04040_b200 import build as ls_build
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+@pytest.fixture(scope="module")
+def lib():
+    ls_build.build()
+    return ls.lib()
+
+
+def _declared_in_header():
+    text = (ROOT / "include" / "ls.h").read_text()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(ls_[a-z_]+)\s*\(", text)))
+
+
+def test_header_symbols_exported(lib):
+    declared = _declared_in_header()
+    assert declared == sorted(ls.SYMBOLS), "binding.SYMBOLS must list exactly what ls.h declares"
+    for name in declared:
+        assert getattr(lib, name) is not None
+
+
+def test_status_strings(lib):
+    names = ["LS_OK", "LS_ERR_ARG", "LS_ERR_DIM", "LS_ERR_DTYPE", "LS_ERR_ALLOC", "LS_ERR_CUDA", "LS_ERR_CAPACITY",
+             "LS_NOT_CONVERGED", "LS_ERR_STATE"]
+    for code, name in enumerate(names):
+        assert lib.ls_status_str(code).decode() == name
+    assert lib.ls_status_str(99).decode() == "LS_UNKNOWN"
+
+
+def test_params_struct_layout():
+    assert C.sizeof(ls.ls_params) == 48
+    assert ls.ls_params.iters.offset == 40 and ls.ls_params.rebuild.offset == 44
+
+
+def test_bad_arguments_rejected_before_cuda(lib):
+    out = C.c_void_p()
+    assert lib.ls_create(0, 8, 8, ls.LS_F32, None, C.byref(out)) == ls.LS_ERR_DIM
+    assert lib.ls_create(8, 8, -1, ls.LS_F32, None, C.byref(out)) == ls.LS_ERR_DIM
+    assert lib.ls_create(8, 8, 8, 7, None, C.byref(out)) == ls.LS_ERR_DTYPE
+    assert lib.ls_create(8, 8, 8, ls.LS_F32, None, None) == ls.LS_ERR_ARG
+    assert lib.ls_create(1 << 14, 1 << 14, 1 << 14, ls.LS_F32, None, C.byref(out)) == ls.LS_ERR_DIM
+    # null ctx
+    p = ls.make_params(1.0, 0.1, 0.1, 1.0, 2.0, 1)
+    assert lib.ls_step(None, None, None, C.byref(p), 1) == ls.LS_ERR_ARG
+    assert lib.ls_build_band(None, None, 1.0, 1.0) == ls.LS_ERR_ARG
+    assert lib.ls_destroy(None) == ls.LS_OK
+
+
+def test_no_device_fails_loudly(lib):
+    """On a box without a GPU the library must report LS_ERR_CUDA, never compute on the CPU."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    out = C.c_void_p()
+    assert lib.ls_create(8, 8, 8, ls.LS_F32, None, C.byref(out)) == ls.LS_ERR_CUDA
+    assert out.value is None
+    assert lib.ls_last_cuda_error().decode() != ""
+    with pytest.raises(ls.LsError):
+        ls.ls_create(8, 8, 8, ls.LS_F32)
+
+
+def test_product_does_not_import_oracle():
+    """The product package never references oracle/ (the oracle is test infrastructure)."""
+    pkg = ROOT / "paper_1612_04040_b200"
+    for path in list(pkg.rglob("*.py")) + list(pkg.rglob("*.cu")) + list(pkg.rglob("*.h")):
+        text = path.read_text()
+        assert "import oracle" not in text and "from oracle" not in text and "ls_oracle" not in text, path
+        assert "liboracle" not in text, path

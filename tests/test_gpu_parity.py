@@ -1,0 +1,311 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Band masks / brick lists bit-exact; fields within the north_star
+tolerances (1e-5*dx per step fp32, 1e-12*dx fp64).  Sizes span several bricks and ragged tails.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import ls_oracle as orc
+from paper_1612_04040_b200 import binding as ls
+from paper_1612_04040_b200 import inputs
+
+from gpu_util import Ctx, assert_band_equal, max_err_dx, to_dev, tol_for
+
+pytestmark = pytest.mark.gpu
+INF = float("inf")
+
+
+def _random_band_field(shape, dtype, seed, dx):
+    """A smooth two-signed field with |grad| ~ 1 plus seeded noise: several disconnected band pieces
+    that touch the domain boundary."""
+    nz, ny, nx = shape
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    u = inputs.uniform01(seed, 0, nx * ny * nz).reshape(shape)
+    phi = dx * (4.0 * np.sin(0.37 * x + 0.2) + 3.0 * np.cos(0.29 * y) + 3.5 * np.sin(0.23 * z + 1.0)
+                + 0.8 * (u - 0.5))
+    F = 2.0 * inputs.uniform01(seed + 1, 0, nx * ny * nz).reshape(shape) - 1.0
+    return phi.astype(dtype), F.astype(dtype)
+
+
+SHAPES = [(4, 4, 4), (9, 13, 20), (17, 8, 33), (24, 40, 56), (64, 64, 64)]
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("shape", SHAPES)
+def test_build_band_bit_exact(shape, dtype):
+    dx = 1.0 / 32
+    phi, _ = _random_band_field(shape, dtype, 11, dx)
+    gamma = 3 * dx
+    with Ctx(shape, dtype) as ctx:
+        ls.ls_build_band(ctx, to_dev(phi), dx, gamma)
+        assert_band_equal(ctx, phi, gamma)
+
+
+def test_build_band_edge_cases():
+    dx = 0.25
+    shape = (10, 10, 10)
+    with Ctx(shape, np.float32) as ctx:
+        # empty band
+        phi = np.full(shape, 5.0, np.float32)
+        ls.ls_build_band(ctx, to_dev(phi), dx, 1.0)
+        assert ls.ls_band_counts(ctx) == (0, 0, 0, 0)
+        T_ids, T_w, N_ids, N_w = ls.ls_band_export(ctx)
+        assert len(T_ids) == 0 and len(N_ids) == 0
+        # |phi| == gamma is NOT in T (strict <, eq. 6)
+        phi = np.full(shape, 1.0, np.float32)
+        ls.ls_build_band(ctx, to_dev(phi), dx, 1.0)
+        assert ls.ls_band_counts(ctx) == (0, 0, 0, 0)
+        # single point: N is its 7-point star
+        phi[3, 7, 8] = 0.5          # (k, j, i): sits at a brick corner in x (i = 8)
+        ls.ls_build_band(ctx, to_dev(phi), dx, 1.0)
+        assert_band_equal(ctx, phi, 1.0)
+        assert ls.ls_band_counts(ctx)[:2] == (1, 7)
+        # gamma = +inf: every point in T and N, all bricks listed
+        ls.ls_build_band(ctx, to_dev(phi), dx, INF)
+        nT, nN, bT, bN = ls.ls_band_counts(ctx)
+        assert (nT, nN, bT, bN) == (1000, 1000, 8, 8)
+        assert_band_equal(ctx, phi, INF)
+
+
+def test_worked_4x4x4_masks():
+    """SURVEY/DESIGN I13: T and N mask words of the 4^3 worked example (tests/golden/worked_4x4x4.txt)."""
+    i, j, k = np.meshgrid(np.arange(4), np.arange(4), np.arange(4), indexing="ij")
+    phi_ijk = 1.5 * i - 0.5 * j * j + 0.25 * j * k + k - 2.25
+    phi = np.ascontiguousarray(phi_ijk.transpose(2, 1, 0)).astype(np.float64)  # (k, j, i)
+    with Ctx((4, 4, 4), np.float64) as ctx:
+        ls.ls_build_band(ctx, to_dev(phi), 1.0, 3.0)
+        nT, nN, bT, bN = ls.ls_band_counts(ctx)
+        assert (nT, nN, bT, bN) == (45, 60, 1, 1)
+        _, T_w, _, N_w = ls.ls_band_export(ctx)
+        assert [hex(int(w)) for w in T_w[0][:4]] == ["0x80e0f0f", "0xc0f0707", "0xe070707", "0x7030303"]
+        assert [hex(int(w)) for w in N_w[0][:4]] == ["0xe0f0f0f", "0xf0f0f0f", "0xf0f0f0f", "0xf070707"]
+        assert not T_w[0][4:].any() and not N_w[0][4:].any()
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("shape", SHAPES[1:])
+def test_advance_band_parity(shape, dtype):
+    dx = 1.0 / 32
+    phi, F = _random_band_field(shape, dtype, 21, dx)
+    gamma, beta, dt = 4 * dx, 2 * dx, 0.4 * dx
+    Tm, _ = orc.band_masks(phi, gamma)
+    want = orc.advance(phi, F, Tm, dt, dx, beta, gamma)
+    with Ctx(shape, dtype) as ctx:
+        d_phi, d_F = to_dev(phi), to_dev(F)
+        out = torch.empty_like(d_phi)
+        ls.ls_build_band(ctx, d_phi, dx, gamma)
+        ls.ls_advance(ctx, d_phi, d_F, dt, dx, beta, gamma, out)
+        got = out.cpu().numpy()
+    assert max_err_dx(got, want, dx) <= tol_for(dtype)
+    assert np.array_equal(got, want), "advance is expected to be bit-identical to the oracle (exact mode)"
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("shape", [(9, 13, 20), (32, 32, 32), (40, 24, 72)])
+def test_advance_dense_parity(shape, dtype):
+    dx = 1.0 / 32
+    phi, F = _random_band_field(shape, dtype, 31, dx)
+    dt = 0.4 * dx
+    want = orc.advance(phi, F, None, dt, dx, INF, INF)
+    with Ctx(shape, dtype) as ctx:
+        d_phi, d_F = to_dev(phi), to_dev(F)
+        out = torch.empty_like(d_phi)
+        ls.ls_advance(ctx, d_phi, d_F, dt, dx, INF, INF, out)   # no band needed in full-domain mode
+        got = out.cpu().numpy()
+    assert max_err_dx(got, want, dx) <= tol_for(dtype)
+    assert np.array_equal(got, want)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("iters", [0, 1, 2, 5])
+def test_reinit_parity(iters, dtype):
+    shape = (24, 40, 56)
+    dx = 1.0 / 32
+    phi, _ = _random_band_field(shape, dtype, 41, dx)
+    gamma, dtau = 4 * dx, 0.5 * dx
+    _, Nm = orc.band_masks(phi, gamma)
+    want = orc.reinit(phi, Nm, dtau, dx, gamma, iters)
+    with Ctx(shape, dtype) as ctx:
+        d_phi = to_dev(phi)
+        d = torch.empty_like(d_phi)
+        ls.ls_build_band(ctx, d_phi, dx, gamma)
+        ls.ls_reinit(ctx, d, d_phi, dtau, dx, gamma, iters)
+        got = d.cpu().numpy()
+    assert max_err_dx(got, want, dx) <= tol_for(dtype) * max(iters, 1)
+    assert np.array_equal(got, want)
+    assert np.all(np.abs(got) <= np.asarray(gamma, dtype))          # eq. 10 everywhere
+
+
+def test_reinit_zero_stays_zero():
+    """I11: points with d == 0 never move (S = 0, R12)."""
+    shape = (16, 16, 16)
+    dx = 1.0 / 16
+    phi, _ = _random_band_field(shape, np.float32, 51, dx)
+    phi[4:12, 5, 3:9] = 0.0
+    with Ctx(shape, np.float32) as ctx:
+        d_phi = to_dev(phi)
+        d = torch.empty_like(d_phi)
+        ls.ls_build_band(ctx, d_phi, dx, 3 * dx)
+        ls.ls_reinit(ctx, d, d_phi, 0.5 * dx, dx, 3 * dx, 7)
+        got = d.cpu().numpy()
+    assert np.all(got[4:12, 5, 3:9] == 0.0)
+
+
+def _run_steps(w, n_steps, rebuild, chunks=1):
+    """GPU free-running: n_steps split into `chunks` ls_step calls."""
+    with Ctx(w.shape, w.dtype) as ctx:
+        d_phi, d_F = to_dev(w.phi), to_dev(w.F)
+        p = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild)
+        per = n_steps // chunks
+        for c in range(chunks):
+            ls.ls_step(ctx, d_phi, d_F, p, per if c < chunks - 1 else n_steps - per * (chunks - 1))
+        updates, steps, launches = ls.ls_stats(ctx)
+        band = ls.ls_band_export(ctx)
+        return d_phi.cpu().numpy(), updates, steps, band
+
+
+@pytest.mark.parametrize("rebuild", [ls.LS_REBUILD_FULL, ls.LS_REBUILD_INCREMENTAL])
+def test_step_cfg1_free_running(rebuild):
+    """cfg 1 (64^3 sphere, F = 1, 10 steps x 5 reinit): final field, update count, last band."""
+    w = inputs.config(1)
+    want, upd = orc.step(w.phi, w.F, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, w.n_steps)
+    got, updates, steps, band = _run_steps(w, w.n_steps, rebuild)
+    assert steps == w.n_steps and updates == upd
+    assert max_err_dx(got, want, w.dx) <= TOL * w.n_steps
+    assert np.array_equal(got, want), "exact mode: free-running field is bit-identical"
+    # the band the last step used is the band of phi^{n_steps-1}
+    prev, _ = orc.step(w.phi, w.F, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, w.n_steps - 1)
+    Tm, Nm = orc.band_masks(prev, w.gamma)
+    T_ids, T_w, _ = orc.brick_list(Tm)
+    N_ids, N_w, _ = orc.brick_list(Nm)
+    assert np.array_equal(band[0], T_ids) and np.array_equal(band[1], T_w)
+    assert np.array_equal(band[2], N_ids) and np.array_equal(band[3], N_w)
+
+
+TOL = 1e-5
+
+
+@pytest.mark.parametrize("rebuild", [ls.LS_REBUILD_FULL, ls.LS_REBUILD_INCREMENTAL])
+@pytest.mark.parametrize("iters", [0, 1, 2, 5])
+def test_step_teacher_forced_cfg3(iters, rebuild):
+    """cfg 3 shape at 96^3 (spheres cross the boundary, two-signed F): every step restarts from the
+    oracle's phi^n; the band and phi^{n+1} are compared each step."""
+    w = inputs.config(3, n=96)
+    phi = w.phi
+    with Ctx(w.shape, w.dtype) as ctx:
+        d_F = to_dev(w.F)
+        p = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, iters, rebuild)
+        for s in range(4):
+            d_phi = to_dev(phi)
+            ls.ls_step(ctx, d_phi, d_F, p, 1)
+            assert_band_equal(ctx, phi, w.gamma)
+            want, _ = orc.step(phi, w.F, w.dx, w.dt, w.dtau, w.beta, w.gamma, iters, 1)
+            got = d_phi.cpu().numpy()
+            assert max_err_dx(got, want, w.dx) <= TOL, f"step {s}"
+            assert np.array_equal(got, want), f"step {s}"
+            phi = want
+
+
+@pytest.mark.parametrize("rebuild", [ls.LS_REBUILD_FULL, ls.LS_REBUILD_INCREMENTAL])
+@pytest.mark.parametrize("cfg,n,steps", [(3, 96, 12), (4, 128, 12), (1, 40, 6)])
+def test_step_free_running_multi(cfg, n, steps, rebuild):
+    """Several steps inside one ls_step call and across two calls (scratch-buffer consistency)."""
+    w = inputs.config(cfg, n=n)
+    want, upd = orc.step(w.phi, w.F, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, steps)
+    for chunks in (1, 2):
+        got, updates, nsteps, _ = _run_steps(w, steps, rebuild, chunks)
+        assert nsteps == steps and updates == upd
+        assert max_err_dx(got, want, w.dx) <= TOL * steps
+        assert np.array_equal(got, want)
+        assert np.all(np.abs(got) <= np.float32(w.gamma))
+
+
+def test_step_ragged_fp64():
+    """Non-multiple-of-8 dims (paper-shaped 101-style grid, scaled down), fp64, even and odd iters."""
+    shape = (21, 37, 50)
+    dx = 1.0 / 32
+    phi, F = _random_band_field(shape, np.float64, 61, dx)
+    F *= 0.5
+    for iters in (2, 3):
+        want, upd = orc.step(phi, F, dx, 0.4 * dx, 0.5 * dx, 2 * dx, 4 * dx, iters, 5)
+        for rebuild in (ls.LS_REBUILD_FULL, ls.LS_REBUILD_INCREMENTAL):
+            with Ctx(shape, np.float64) as ctx:
+                d_phi, d_F = to_dev(phi), to_dev(F)
+                ls.ls_step(ctx, d_phi, d_F, ls.make_params(dx, 0.4 * dx, 0.5 * dx, 2 * dx, 4 * dx, iters, rebuild), 5)
+                got = d_phi.cpu().numpy()
+                assert ls.ls_stats(ctx)[0] == upd
+            assert max_err_dx(got, want, dx) <= 1e-12 * 5
+            assert np.array_equal(got, want)
+
+
+def test_step_host_matches_device():
+    w = inputs.config(1, n=32)
+    p = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters)
+    want, _ = orc.step(w.phi, w.F, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, 3)
+    host_phi = w.phi.copy()
+    with Ctx(w.shape, w.dtype) as ctx:
+        ls.ls_step_host(ctx, host_phi, w.F, p, 3)
+    assert np.array_equal(host_phi, want)
+
+
+def test_dense_cfg2_steps():
+    """cfg 2 at 64^3 and three steps at the full 256^3: ping-pong of full-domain advances."""
+    for n, steps in ((64, 10), (256, 3)):
+        w = inputs.config(2, n=n)
+        a = w.phi
+        for _ in range(steps):
+            a = orc.advance(a, w.F, None, w.dt, w.dx, INF, INF)
+        with Ctx(w.shape, w.dtype) as ctx:
+            x, y, d_F = to_dev(w.phi), torch.empty_like(to_dev(w.phi)), to_dev(w.F)
+            for _ in range(steps):
+                ls.ls_advance(ctx, x, d_F, w.dt, w.dx, INF, INF, y)
+                x, y = y, x
+            got = x.cpu().numpy()
+            assert ls.ls_stats(ctx)[0] == steps * n ** 3
+        assert max_err_dx(got, a, w.dx) <= TOL * steps
+        assert np.array_equal(got, a)
+
+
+def test_cfg5_reinit_tol():
+    """cfg 5 shape at 64^3 fp64: (i) trajectory parity over the first 300 iterations, (ii) the stopping
+    rule (same iteration count and residual as the oracle for a loose tol), (iii) windowed parity
+    from a GPU checkpoint, (iv) fixed-point certificate."""
+    w = inputs.config(5, n=64)
+    _, Nm = orc.band_masks(w.phi, w.gamma)
+    with Ctx(w.shape, w.dtype) as ctx:
+        d_phi = to_dev(w.phi)
+        d = torch.empty_like(d_phi)
+        ls.ls_build_band(ctx, d_phi, w.dx, w.gamma)
+        assert_band_equal(ctx, w.phi, w.gamma)
+        # (i)
+        ls.ls_reinit(ctx, d, d_phi, w.dtau, w.dx, w.gamma, 300)
+        want = orc.reinit(w.phi, Nm, w.dtau, w.dx, w.gamma, 300)
+        got = d.cpu().numpy()
+        assert max_err_dx(got, want, w.dx) <= 1e-12 * 300
+        assert np.array_equal(got, want)
+        # (ii)
+        tol = 2e-4 * w.dx
+        k, r, conv = ls.ls_reinit_tol(ctx, d, d_phi, w.dtau, w.dx, w.gamma, tol, 5000, 10)
+        d_or, k_or, r_or, conv_or = orc.reinit_tol(w.phi, w.dtau, w.dx, w.gamma, tol, 5000, 10)
+        assert conv and conv_or and k == k_or and r == r_or
+        g_conv = d.cpu().numpy()
+        assert np.array_equal(g_conv, d_or)
+        # not converged path
+        k2, r2, conv2 = ls.ls_reinit_tol(ctx, d, d_phi, w.dtau, w.dx, w.gamma, 1e-30, 37, 10)
+        assert (k2, conv2) == (37, False)
+        d37 = orc.reinit(w.phi, Nm, w.dtau, w.dx, w.gamma, 37)
+        assert np.array_equal(d.cpu().numpy(), d37)
+        # (iii) windowed: continue both sides for 50 iterations from the GPU state at k (unclamped
+        # inside N; the clamp only touched points with |d| > gamma, so restart from the clamped field
+        # on both sides with the ORIGINAL N)
+        chk = d_or.copy()
+        want50 = orc.reinit(chk, Nm, w.dtau, w.dx, w.gamma, 50)
+        d2 = torch.empty_like(d_phi)
+        ls.ls_reinit(ctx, d2, to_dev(chk), w.dtau, w.dx, w.gamma, 50)   # band in ctx is still N(phi0)
+        assert np.array_equal(d2.cpu().numpy(), want50)
+        # (iv) certificate: one oracle iteration on the GPU's converged state moves it by < tol
+        # (checked away from the rim, where the final eq. 10 clamp has altered the iterate)
+        nxt, _ = orc.reinit_iter(g_conv, Nm, w.dtau, w.dx)
+        inner = (Nm != 0) & (np.abs(g_conv) < w.gamma - 2 * w.dx)
+        assert np.max(np.abs(nxt - g_conv)[inner]) < tol
