@@ -65,7 +65,25 @@ typedef struct {
     double gamma; /* tube half-width: T = {|phi| < gamma}         (eq. 6); 0 < beta < gamma */
     int32_t iters;   /* reinitialisation iterations per step, >= 0 (R13) */
     int32_t rebuild; /* ls_rebuild */
+    int32_t chained; /* 0 or 1.  1 = the caller promises that `phi` is the same buffer, unmodified, that
+                        the previous ls_step on this ctx returned (same gamma), and that no other band
+                        call was made on the ctx in between.  The ctx then keeps its band, its scratch
+                        field and (LS_REBUILD_INCREMENTAL) the T masks it emitted from phi^n, so the call
+                        does no whole-grid work at all: no resync copy, no scan, no global clamp.  If the
+                        ctx cannot verify pointer / gamma / state it silently runs the unchained path. */
+    int32_t reserved; /* must be 0 */
 } ls_params;
+
+/* Kernel classes of the per-kernel device timing (ls_profile_*). */
+typedef enum {
+    LS_K_CLASSIFY = 0, /* whole-grid |phi| < gamma sweep of Step 1 */
+    LS_K_BAND = 1,     /* dilation + ordered compaction of the brick lists */
+    LS_K_ADVANCE = 2,  /* Step 2 */
+    LS_K_REINIT = 3,   /* one Step 3 sweep (clamp / T emission fused into the last) */
+    LS_K_CLAMP = 4,    /* eq. 10 passes outside the reinit sweeps */
+    LS_K_COPY = 5,     /* whole-field device copies (resync of the scratch field) */
+    LS_K_KINDS = 6
+} ls_kernel_kind;
 
 typedef struct ls_ctx ls_ctx;
 
@@ -140,6 +158,15 @@ ls_status ls_step_host(ls_ctx* ctx, void* phi_host, const void* F_host, const ls
  * kernels launched by this ctx.  HOST out-pointers, any may be NULL.  Synchronises. */
 ls_status ls_stats(ls_ctx* ctx, int64_t* point_updates, int64_t* steps, int64_t* kernel_launches);
 ls_status ls_stats_reset(ls_ctx* ctx);
+
+/* Per-kernel device timing.  While enabled, every launch (or launch group, for LS_K_BAND) this ctx
+ * enqueues is bracketed by two CUDA events on the ctx stream; ls_profile_read synchronises and returns
+ * the summed elapsed time (milliseconds) and the number of bracketed launches of one ls_kernel_kind
+ * since the last ls_profile_reset / enable.  HOST out-pointers, either may be NULL.  The events cost a
+ * few microseconds per launch: headline timings are taken with profiling off. */
+ls_status ls_profile_enable(ls_ctx* ctx, int32_t on);
+ls_status ls_profile_read(ls_ctx* ctx, int32_t kind, double* ms_total, int64_t* launches);
+ls_status ls_profile_reset(ls_ctx* ctx);
 
 #ifdef __cplusplus
 }

@@ -19,18 +19,21 @@ LS_OK, LS_ERR_ARG, LS_ERR_DIM, LS_ERR_DTYPE, LS_ERR_ALLOC, LS_ERR_CUDA, LS_ERR_C
     LS_ERR_STATE = range(9)
 LS_F32, LS_F64 = 0, 1
 LS_REBUILD_FULL, LS_REBUILD_INCREMENTAL = 0, 1
+LS_K_CLASSIFY, LS_K_BAND, LS_K_ADVANCE, LS_K_REINIT, LS_K_CLAMP, LS_K_COPY, LS_K_KINDS = range(7)
+KERNEL_KINDS = ("classify", "band", "advance", "reinit", "clamp", "copy")
 
 # every symbol include/ls.h declares (tests/test_abi.py checks the library exports them all)
 SYMBOLS = (
     "ls_status_str", "ls_last_cuda_error", "ls_create", "ls_destroy", "ls_build_band", "ls_band_counts",
     "ls_band_export", "ls_advance", "ls_reinit", "ls_reinit_tol", "ls_step", "ls_step_host", "ls_stats",
-    "ls_stats_reset",
+    "ls_stats_reset", "ls_profile_enable", "ls_profile_read", "ls_profile_reset",
 )
 
 
 class ls_params(C.Structure):
     _fields_ = [("dx", C.c_double), ("dt", C.c_double), ("dtau", C.c_double), ("beta", C.c_double),
-                ("gamma", C.c_double), ("iters", C.c_int32), ("rebuild", C.c_int32)]
+                ("gamma", C.c_double), ("iters", C.c_int32), ("rebuild", C.c_int32),
+                ("chained", C.c_int32), ("reserved", C.c_int32)]
 
 
 class LsError(RuntimeError):
@@ -70,6 +73,9 @@ def lib() -> C.CDLL:
         L.ls_step_host.argtypes = [_P, _P, _P, C.POINTER(ls_params), _I]
         L.ls_stats.argtypes = [_P, C.POINTER(_L), C.POINTER(_L), C.POINTER(_L)]
         L.ls_stats_reset.argtypes = [_P]
+        L.ls_profile_enable.argtypes = [_P, _I]
+        L.ls_profile_read.argtypes = [_P, _I, C.POINTER(_D), C.POINTER(_L)]
+        L.ls_profile_reset.argtypes = [_P]
         for name in SYMBOLS[2:]:
             getattr(L, name).restype = C.c_int
         _lib = L
@@ -155,8 +161,8 @@ def ls_reinit_tol(ctx: int, d, phi_bar, dtau: float, dx: float, gamma: float, to
     return k.value, r.value, st == LS_OK
 
 
-def make_params(dx, dt, dtau, beta, gamma, iters, rebuild=LS_REBUILD_FULL) -> ls_params:
-    return ls_params(dx, dt, dtau, beta, gamma, iters, rebuild)
+def make_params(dx, dt, dtau, beta, gamma, iters, rebuild=LS_REBUILD_FULL, chained=0) -> ls_params:
+    return ls_params(dx, dt, dtau, beta, gamma, iters, rebuild, chained, 0)
 
 
 def ls_step(ctx: int, phi, F, p: ls_params, n_steps: int) -> None:
@@ -176,3 +182,18 @@ def ls_stats(ctx: int):
 
 def ls_stats_reset(ctx: int) -> None:
     _ck(lib().ls_stats_reset(_P(ctx)), "ls_stats_reset")
+
+
+def ls_profile_enable(ctx: int, on: bool) -> None:
+    _ck(lib().ls_profile_enable(_P(ctx), int(bool(on))), "ls_profile_enable")
+
+
+def ls_profile_read(ctx: int, kind: int):
+    """-> (ms_total, launches) of one ls_kernel_kind"""
+    ms, n = _D(), _L()
+    _ck(lib().ls_profile_read(_P(ctx), kind, C.byref(ms), C.byref(n)), "ls_profile_read")
+    return ms.value, n.value
+
+
+def ls_profile_reset(ctx: int) -> None:
+    _ck(lib().ls_profile_reset(_P(ctx)), "ls_profile_reset")

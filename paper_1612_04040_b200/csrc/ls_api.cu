@@ -7,6 +7,7 @@
 #include <cstring>
 #include <limits>
 #include <new>
+#include <vector>
 
 #include "../../include/ls.h"
 #include "ls_internal.h"
@@ -29,6 +30,17 @@ struct ls_ctx {
     int64_t dense_updates;
     size_t elem;          // sizeof field element
     int64_t n;            // nx*ny*nz
+    // chained stepping (ls_params::chained): what the last ls_step left behind
+    const void* chain_phi;   // phi buffer the ctx state is consistent with (null: none)
+    double chain_gamma;
+    bool chain_have_T;       // tmask / flagT already hold the T masks of the current phi
+    // per-kernel device timing (ls_profile_*)
+    bool prof_on;
+    struct ProfRec { int kind; cudaEvent_t a, b; };
+    std::vector<ProfRec>* prof_recs;    // brackets recorded since the last read
+    std::vector<cudaEvent_t>* prof_pool;  // idle events
+    double prof_ms[LS_K_KINDS];
+    int64_t prof_n[LS_K_KINDS];
 };
 
 namespace {
@@ -51,6 +63,48 @@ ls_status cuda_fail(cudaError_t e, const char* what) {
         cudaError_t e_ = cudaPeekAtLastError();                          \
         if (e_ != cudaSuccess) { cudaGetLastError(); return cuda_fail(e_, "kernel launch"); } \
     } while (0)
+
+// Bracket the launches enqueued during its lifetime with two events on the ctx stream.
+struct ProfScope {
+    ls_ctx* c;
+    ls_ctx::ProfRec r;
+    bool live;
+    ProfScope(ls_ctx* ctx, int kind) : c(ctx), live(false) {
+        if (!c->prof_on) return;
+        auto get = [&](cudaEvent_t* e) {
+            if (!c->prof_pool->empty()) { *e = c->prof_pool->back(); c->prof_pool->pop_back(); return true; }
+            return cudaEventCreate(e) == cudaSuccess;
+        };
+        r.kind = kind;
+        if (!get(&r.a)) return;
+        if (!get(&r.b)) { c->prof_pool->push_back(r.a); return; }
+        cudaEventRecord(r.a, c->stream);
+        live = true;
+    }
+    ~ProfScope() {
+        if (!live) return;
+        cudaEventRecord(r.b, c->stream);
+        c->prof_recs->push_back(r);
+    }
+};
+
+// Fold finished brackets into the totals.  Synchronises the stream.
+ls_status prof_collect(ls_ctx* c) {
+    if (c->prof_recs->empty()) return LS_OK;
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    for (auto& r : *c->prof_recs) {
+        float ms = 0.f;
+        if (e == cudaSuccess && cudaEventElapsedTime(&ms, r.a, r.b) == cudaSuccess) {
+            c->prof_ms[r.kind] += ms;
+            c->prof_n[r.kind] += 1;
+        }
+        c->prof_pool->push_back(r.a);
+        c->prof_pool->push_back(r.b);
+    }
+    c->prof_recs->clear();
+    if (e != cudaSuccess) return cuda_fail(e, "ls_profile: cudaStreamSynchronize");
+    return LS_OK;
+}
 
 template <typename T>
 ls::StencilParams<T> make_params(double dx, double dt, double beta, double gamma) {
@@ -83,12 +137,16 @@ bool bad_band_params(double dx, double beta, double gamma) {
 
 ls_status build_band_impl(ls_ctx* c, const void* phi, double gamma, int iters, bool count_step, bool classify) {
     if (classify) {
+        ProfScope ps(c, LS_K_CLASSIFY);
         if (c->dtype == LS_F32)
             ls::launch_classify<float>((const float*)phi, c->g, (float)gamma, c->bb, c->stream, &c->launches);
         else
             ls::launch_classify<double>((const double*)phi, c->g, gamma, c->bb, c->stream, &c->launches);
     }
-    ls::launch_dilate_compact(c->g, c->bb, iters, count_step, c->stream, &c->launches);
+    {
+        ProfScope ps(c, LS_K_BAND);
+        ls::launch_dilate_compact(c->g, c->bb, iters, count_step, c->stream, &c->launches);
+    }
     LS_CK_LAUNCH();
     c->band_valid = true;
     return LS_OK;
@@ -103,31 +161,50 @@ ls_status step_impl(ls_ctx* c, T* phi, const T* F, const ls_params* p, int n_ste
     const ls::StencilParams<T> rei = make_params<T>(p->dx, p->dtau, p->beta, p->gamma);
     const T gammaT = (T)p->gamma;
     cudaStream_t s = c->stream;
-    // Both Jacobi buffers must agree off the band: start from a full copy, and forget the previous
-    // call's N (the U list is then just N in the first step).
-    LS_CK(cudaMemcpyAsync(S, phi, (size_t)c->n * sizeof(T), cudaMemcpyDeviceToDevice, s));
-    LS_CK(cudaMemsetAsync(c->bb.flagNprev, 0, (size_t)c->g.nbricks, s));
-    bool have_T = false;  // T masks of phi^n already emitted by the previous step's last sweep
+    // chained: the ctx state (S consistent with phi off the band, flagNprev = N of the last step,
+    // phi clamped everywhere) carries over from the previous call.
+    const bool chained = p->chained && c->chain_phi == (const void*)phi && c->chain_gamma == p->gamma;
+    bool have_T = chained && c->chain_have_T && p->rebuild == LS_REBUILD_INCREMENTAL;
+    c->chain_phi = nullptr;   // re-established only when the whole call was enqueued
+    if (!chained) {
+        // Both Jacobi buffers must agree off the band: start from a full copy, and forget the previous
+        // call's N (the U list is then just N in the first step).
+        ProfScope ps(c, LS_K_COPY);
+        LS_CK(cudaMemcpyAsync(S, phi, (size_t)c->n * sizeof(T), cudaMemcpyDeviceToDevice, s));
+        LS_CK(cudaMemsetAsync(c->bb.flagNprev, 0, (size_t)c->g.nbricks, s));
+    }
     for (int step = 0; step < n_steps; ++step) {
         st = build_band_impl(c, phi, p->gamma, p->iters, true, !have_T);   // Step 1
         if (st != LS_OK) return st;
-        ls::launch_advance_band<T>(phi, F, S, c->g, adv, c->bb, false, s, &c->launches);   // Step 2: phi -> S
-        const bool emit = p->rebuild == LS_REBUILD_INCREMENTAL && step + 1 < n_steps && (p->iters & 1);
+        {
+            ProfScope ps(c, LS_K_ADVANCE);
+            ls::launch_advance_band<T>(phi, F, S, c->g, adv, c->bb, false, s, &c->launches);   // Step 2: phi -> S
+        }
+        // T masks of phi^{n+1} come out of the last sweep (the one that writes phi): odd iters only
+        const bool emit = p->rebuild == LS_REBUILD_INCREMENTAL && (p->iters & 1);
         T* src = S;
         T* dst = phi;
         for (int it = 0; it < p->iters; ++it) {                             // Step 3
             const bool last = it == p->iters - 1;
+            ProfScope ps(c, LS_K_REINIT);
             ls::launch_reinit_band<T>(src, dst, c->g, rei, c->bb, last, nullptr, emit && last, s, &c->launches);
             T* t = src; src = dst; dst = t;
         }
-        if (src != phi)  // even iters: the result sits in S
+        if (src != phi) {  // even iters: the result sits in S
+            ProfScope ps(c, LS_K_CLAMP);
             ls::launch_copy_clamp_band<T>(S, phi, c->g, gammaT, c->bb, s, &c->launches);
-        if (step == 0)   // eq. 10 at every point (R14); afterwards points off N already hold +-gamma
+        }
+        if (step == 0 && !chained) {  // eq. 10 at every point (R14); afterwards points off N already hold +-gamma
+            ProfScope ps(c, LS_K_CLAMP);
             ls::launch_clamp_all<T>(phi, S, c->n, gammaT, s, &c->launches);
+        }
         LS_CK_LAUNCH();
         have_T = emit;
         uint8_t* t = c->bb.flagN; c->bb.flagN = c->bb.flagNprev; c->bb.flagNprev = t;
     }
+    c->chain_phi = phi;
+    c->chain_gamma = p->gamma;
+    c->chain_have_T = have_T;
     return LS_OK;
 }
 
@@ -136,6 +213,7 @@ ls_status check_step_args(ls_ctx* c, const void* phi, const void* F, const ls_pa
     if (n_steps < 0 || p->iters < 0) return LS_ERR_ARG;
     if (!(p->dx > 0) || !(p->beta > 0) || !(p->beta < p->gamma) || std::isinf(p->gamma)) return LS_ERR_ARG;
     if (p->rebuild != LS_REBUILD_FULL && p->rebuild != LS_REBUILD_INCREMENTAL) return LS_ERR_ARG;
+    if ((p->chained != 0 && p->chained != 1) || p->reserved != 0) return LS_ERR_ARG;
     return LS_OK;
 }
 
@@ -178,6 +256,9 @@ ls_status ls_create(int32_t nx, int32_t ny, int32_t nz, ls_dtype dtype, void* cu
     c->stream = (cudaStream_t)cuda_stream;
     c->elem = dtype == LS_F32 ? 4 : 8;
     c->n = (int64_t)nx * ny * nz;
+    c->prof_recs = new (std::nothrow) std::vector<ls_ctx::ProfRec>();
+    c->prof_pool = new (std::nothrow) std::vector<cudaEvent_t>();
+    if (!c->prof_recs || !c->prof_pool) { delete c->prof_recs; delete c->prof_pool; delete c; return LS_ERR_ALLOC; }
     const int tile = ls::scan_tile();
     const int64_t padded = (nbricks + tile - 1) / tile * tile;
     ls::BandBuffers& bb = c->bb;
@@ -224,6 +305,10 @@ ls_status ls_destroy(ls_ctx* c) {
         if (p) cudaFree(p);
     if (c->host_counts) cudaFreeHost(c->host_counts);
     if (c->host_residual) cudaFreeHost(c->host_residual);
+    for (auto& r : *c->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    for (cudaEvent_t e : *c->prof_pool) cudaEventDestroy(e);
+    delete c->prof_recs;
+    delete c->prof_pool;
     cudaGetLastError();
     delete c;
     return LS_OK;
@@ -232,6 +317,7 @@ ls_status ls_destroy(ls_ctx* c) {
 ls_status ls_build_band(ls_ctx* c, const void* phi, double dx, double gamma) {
     if (!c || !phi) return LS_ERR_ARG;
     if (!(dx > 0) || !(gamma > 0)) return LS_ERR_ARG;
+    c->chain_phi = nullptr;
     LS_CK(cudaMemsetAsync(c->bb.flagNprev, 0, (size_t)c->g.nbricks, c->stream));
     return build_band_impl(c, phi, gamma, 0, false, true);
 }
@@ -268,6 +354,7 @@ ls_status ls_advance(ls_ctx* c, const void* phi, const void* F, double dt, doubl
     const bool dense = std::isinf(beta) && std::isinf(gamma);
     cudaStream_t s = c->stream;
     if (dense) {
+        ProfScope ps(c, LS_K_ADVANCE);
         if (c->dtype == LS_F32)
             ls::launch_advance_dense<float>((const float*)phi, (const float*)F, (float*)out, c->g,
                                             make_params<float>(dx, dt, beta, gamma), s, &c->launches);
@@ -280,7 +367,11 @@ ls_status ls_advance(ls_ctx* c, const void* phi, const void* F, double dt, doubl
     }
     if (!c->band_valid) return LS_ERR_STATE;
     // out = phi everywhere, then eq. 8 on the T bricks.
-    LS_CK(cudaMemcpyAsync(out, phi, (size_t)c->n * c->elem, cudaMemcpyDeviceToDevice, s));
+    {
+        ProfScope ps(c, LS_K_COPY);
+        LS_CK(cudaMemcpyAsync(out, phi, (size_t)c->n * c->elem, cudaMemcpyDeviceToDevice, s));
+    }
+    ProfScope ps(c, LS_K_ADVANCE);
     if (c->dtype == LS_F32)
         ls::launch_advance_band<float>((const float*)phi, (const float*)F, (float*)out, c->g,
                                        make_params<float>(dx, dt, beta, gamma), c->bb, true, s, &c->launches);
@@ -305,8 +396,12 @@ ls_status reinit_impl(ls_ctx* c, T* d, const T* phi_bar, double dtau, double dx,
     cudaStream_t s = c->stream;
     const size_t bytes = (size_t)c->n * sizeof(T);
     const ls::StencilParams<T> rei = make_params<T>(dx, dtau, gamma * 0.5, gamma);
-    LS_CK(cudaMemcpyAsync(d, phi_bar, bytes, cudaMemcpyDeviceToDevice, s));
-    LS_CK(cudaMemcpyAsync(S, phi_bar, bytes, cudaMemcpyDeviceToDevice, s));
+    c->chain_phi = nullptr;   // the scratch field is reused here
+    {
+        ProfScope ps(c, LS_K_COPY);
+        LS_CK(cudaMemcpyAsync(d, phi_bar, bytes, cudaMemcpyDeviceToDevice, s));
+        LS_CK(cudaMemcpyAsync(S, phi_bar, bytes, cudaMemcpyDeviceToDevice, s));
+    }
     const bool to_tol = tol >= 0;
     // fixed count: choose the first source so that the last sweep writes d
     T* src = (!to_tol && (iters & 1)) ? S : d;
@@ -318,8 +413,11 @@ ls_status reinit_impl(ls_ctx* c, T* d, const T* phi_bar, double dtau, double dx,
         ++k;
         const bool check = to_tol && (k % check_every == 0 || k == iters);
         if (check) LS_CK(cudaMemsetAsync(c->residual, 0, 8, s));
-        ls::launch_reinit_band<T>(src, dst, c->g, rei, c->bb, false, check ? c->residual : nullptr, false, s,
-                                  &c->launches);
+        {
+            ProfScope ps(c, LS_K_REINIT);
+            ls::launch_reinit_band<T>(src, dst, c->g, rei, c->bb, false, check ? c->residual : nullptr, false, s,
+                                      &c->launches);
+        }
         T* t = src; src = dst; dst = t;
         if (check) {
             LS_CK_LAUNCH();
@@ -332,8 +430,14 @@ ls_status reinit_impl(ls_ctx* c, T* d, const T* phi_bar, double dtau, double dx,
         }
     }
     LS_CK_LAUNCH();
-    if (src != d) LS_CK(cudaMemcpyAsync(d, src, bytes, cudaMemcpyDeviceToDevice, s));   // result is in `src`
-    ls::launch_clamp_all<T>(d, (T*)nullptr, c->n, (T)gamma, s, &c->launches);          // eq. 10 everywhere
+    if (src != d) {   // result is in `src`
+        ProfScope ps(c, LS_K_COPY);
+        LS_CK(cudaMemcpyAsync(d, src, bytes, cudaMemcpyDeviceToDevice, s));
+    }
+    {
+        ProfScope ps(c, LS_K_CLAMP);
+        ls::launch_clamp_all<T>(d, (T*)nullptr, c->n, (T)gamma, s, &c->launches);          // eq. 10 everywhere
+    }
     LS_CK_LAUNCH();
     if (iters_done) *iters_done = k;
     if (residual_out) *residual_out = r;
@@ -384,8 +488,10 @@ ls_status ls_step_host(ls_ctx* c, void* phi_host, const void* F_host, const ls_p
     LS_CK(cudaMemcpyAsync(c->dev_phi, phi_host, bytes, cudaMemcpyHostToDevice, c->stream));
     LS_CK(cudaMemcpyAsync(c->dev_F, F_host, bytes, cudaMemcpyHostToDevice, c->stream));
     if (n_steps > 0) {
-        st = c->dtype == LS_F32 ? step_impl<float>(c, (float*)c->dev_phi, (const float*)c->dev_F, p, n_steps)
-                                : step_impl<double>(c, (double*)c->dev_phi, (const double*)c->dev_F, p, n_steps);
+        ls_params q = *p;
+        q.chained = 0;   // the staging field was just overwritten
+        st = c->dtype == LS_F32 ? step_impl<float>(c, (float*)c->dev_phi, (const float*)c->dev_F, &q, n_steps)
+                                : step_impl<double>(c, (double*)c->dev_phi, (const double*)c->dev_F, &q, n_steps);
         if (st != LS_OK) return st;
     }
     LS_CK(cudaMemcpyAsync(phi_host, c->dev_phi, bytes, cudaMemcpyDeviceToHost, c->stream));
@@ -401,6 +507,28 @@ ls_status ls_stats(ls_ctx* c, int64_t* point_updates, int64_t* steps, int64_t* k
     if (steps) *steps = (int64_t)c->host_counts->steps;
     if (kernel_launches) *kernel_launches = c->launches;
     return LS_OK;
+}
+
+ls_status ls_profile_enable(ls_ctx* c, int32_t on) {
+    if (!c) return LS_ERR_ARG;
+    c->prof_on = on != 0;
+    return LS_OK;
+}
+
+ls_status ls_profile_read(ls_ctx* c, int32_t kind, double* ms_total, int64_t* launches) {
+    if (!c || kind < 0 || kind >= LS_K_KINDS) return LS_ERR_ARG;
+    ls_status st = prof_collect(c);
+    if (st != LS_OK) return st;
+    if (ms_total) *ms_total = c->prof_ms[kind];
+    if (launches) *launches = c->prof_n[kind];
+    return LS_OK;
+}
+
+ls_status ls_profile_reset(ls_ctx* c) {
+    if (!c) return LS_ERR_ARG;
+    ls_status st = prof_collect(c);
+    for (int k = 0; k < LS_K_KINDS; ++k) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
+    return st;
 }
 
 ls_status ls_stats_reset(ls_ctx* c) {

@@ -41,8 +41,9 @@ def test_status_strings(lib):
 
 
 def test_params_struct_layout():
-    assert C.sizeof(ls.ls_params) == 48
+    assert C.sizeof(ls.ls_params) == 56
     assert ls.ls_params.iters.offset == 40 and ls.ls_params.rebuild.offset == 44
+    assert ls.ls_params.chained.offset == 48 and ls.ls_params.reserved.offset == 52
 
 
 def test_bad_arguments_rejected_before_cuda(lib):

@@ -152,11 +152,11 @@ def test_reinit_zero_stays_zero():
     assert np.all(got[4:12, 5, 3:9] == 0.0)
 
 
-def _run_steps(w, n_steps, rebuild, chunks=1):
+def _run_steps(w, n_steps, rebuild, chunks=1, chained=0):
     """GPU free-running: n_steps split into `chunks` ls_step calls."""
     with Ctx(w.shape, w.dtype) as ctx:
         d_phi, d_F = to_dev(w.phi), to_dev(w.F)
-        p = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild)
+        p = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild, chained)
         per = n_steps // chunks
         for c in range(chunks):
             ls.ls_step(ctx, d_phi, d_F, p, per if c < chunks - 1 else n_steps - per * (chunks - 1))
@@ -213,12 +213,47 @@ def test_step_free_running_multi(cfg, n, steps, rebuild):
     """Several steps inside one ls_step call and across two calls (scratch-buffer consistency)."""
     w = inputs.config(cfg, n=n)
     want, upd = orc.step(w.phi, w.F, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, steps)
-    for chunks in (1, 2):
-        got, updates, nsteps, _ = _run_steps(w, steps, rebuild, chunks)
+    for chunks, chained in ((1, 0), (2, 0), (2, 1), (5, 1)):
+        got, updates, nsteps, _ = _run_steps(w, steps, rebuild, chunks, chained)
         assert nsteps == steps and updates == upd
         assert max_err_dx(got, want, w.dx) <= TOL * steps
         assert np.array_equal(got, want)
         assert np.all(np.abs(got) <= np.float32(w.gamma))
+
+
+def test_step_chained_falls_back_when_phi_differs():
+    """chained = 1 with a different phi buffer (or after another band call) must run the unchained path."""
+    w = inputs.config(1, n=40)
+    want, _ = orc.step(w.phi, w.F, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, 2)
+    p = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, ls.LS_REBUILD_INCREMENTAL, 1)
+    with Ctx(w.shape, w.dtype) as ctx:
+        d_F = to_dev(w.F)
+        a = to_dev(w.phi)
+        ls.ls_step(ctx, a, d_F, p, 2)          # first call: nothing to chain to
+        assert np.array_equal(a.cpu().numpy(), want)
+        b = to_dev(w.phi)                      # another buffer: the promise cannot hold
+        ls.ls_step(ctx, b, d_F, p, 2)
+        assert np.array_equal(b.cpu().numpy(), want)
+        ls.ls_build_band(ctx, b, w.dx, w.gamma)   # a band call in between invalidates the chain
+        want4, _ = orc.step(want, w.F, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, 2)
+        ls.ls_step(ctx, b, d_F, p, 2)
+        assert np.array_equal(b.cpu().numpy(), want4)
+
+
+def test_profile_counts_launches():
+    w = inputs.config(1, n=32)
+    p = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, ls.LS_REBUILD_INCREMENTAL)
+    with Ctx(w.shape, w.dtype) as ctx:
+        d_phi, d_F = to_dev(w.phi), to_dev(w.F)
+        ls.ls_profile_enable(ctx, True)
+        ls.ls_step(ctx, d_phi, d_F, p, 3)
+        got = {name: ls.ls_profile_read(ctx, k) for k, name in enumerate(ls.KERNEL_KINDS)}
+        ls.ls_profile_enable(ctx, False)
+        assert got["reinit"][1] == 15 and got["advance"][1] == 3 and got["band"][1] == 3
+        assert got["classify"][1] == 1 and got["copy"][1] == 1 and got["clamp"][1] == 1
+        assert all(ms > 0 for ms, n in got.values() if n)
+        ls.ls_profile_reset(ctx)
+        assert ls.ls_profile_read(ctx, ls.LS_K_REINIT) == (0.0, 0)
 
 
 def test_step_ragged_fp64():
