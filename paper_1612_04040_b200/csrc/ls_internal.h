@@ -89,6 +89,19 @@ void launch_copy_clamp_band(const T* src, T* dst, const Geom& g, T gamma, const 
 template <typename T>
 void launch_clamp_all(T* a, T* b, int64_t n, T gamma, cudaStream_t s, int64_t* launches);
 
+// ---- TMA-pipelined band kernels (ls_tma.cu) ---------------------------------------------------
+// Usable when every field row starts on a 16-byte boundary (nx*sizeof(T) % 16 == 0, aligned bases) and
+// the driver exposes cuTensorMapEncodeTiled.  The launchers return false (nothing enqueued) if the
+// tensor map cannot be built; the callers then take the scalar kernels of ls_stencil.cu.
+template <typename T>
+bool tma_usable(const Geom& g, const void* a, const void* b, const void* c);
+template <typename T>
+bool launch_reinit_tma(const T* src, T* dst, const Geom& g, const StencilParams<T>& p, const BandBuffers& bb,
+                       bool clamp, unsigned long long* residual, bool emit_T, cudaStream_t s, int64_t* launches);
+template <typename T>
+bool launch_advance_tma(const T* phi, const T* F, T* out, const Geom& g, const StencilParams<T>& p,
+                        const BandBuffers& bb, bool use_T_list, cudaStream_t s, int64_t* launches);
+
 int sm_count();
 
 }  // namespace ls

@@ -6,7 +6,10 @@
 // (this file is compiled with -fmad=false), differences scaled by inv_dx = 1/dx, the six squared
 // terms summed pairwise by axis ((x-pair + y-pair) + z-pair).  Only the gradient norm that the sign
 // of F (or of d) selects is rooted: the other one is multiplied by an exact zero in eq. 3.
+#include <cstdlib>
+
 #include "ls_internal.h"
+#include "ls_math.cuh"
 
 namespace ls {
 
@@ -15,74 +18,6 @@ namespace {
 constexpr int kBandThreads = 256;
 constexpr int kTileEdge = 10;                 // 8 + one halo cell on each side
 constexpr int kTileElems = kTileEdge * kTileEdge * kTileEdge;
-
-template <typename T> __device__ __forceinline__ T pos(T x) { return x > T(0) ? x : T(0); }   // max(x, 0)
-template <typename T> __device__ __forceinline__ T neg(T x) { return x < T(0) ? x : T(0); }   // min(x, 0)
-template <typename T> __device__ __forceinline__ T root(T x);
-template <> __device__ __forceinline__ float root<float>(float x) { return __fsqrt_rn(x); }
-template <> __device__ __forceinline__ double root<double>(double x) { return __dsqrt_rn(x); }
-template <typename T> __device__ __forceinline__ T quot(T a, T b);
-template <> __device__ __forceinline__ float quot<float>(float a, float b) { return __fdiv_rn(a, b); }
-template <> __device__ __forceinline__ double quot<double>(double a, double b) { return __ddiv_rn(a, b); }
-template <typename T> __device__ __forceinline__ T mag(T v);
-template <> __device__ __forceinline__ float mag<float>(float v) { return fabsf(v); }
-template <> __device__ __forceinline__ double mag<double>(double v) { return fabs(v); }
-
-// q+ = (grad+)^2 of eq. 4 and q- = (grad-)^2 of eq. 5 from the 7-point star.
-template <typename T>
-__device__ __forceinline__ void upwind_q(T c, T xm, T xp, T ym, T yp, T zm, T zp, T inv, T& qp, T& qm) {
-    const T Dmx = (c - xm) * inv, Dpx = (xp - c) * inv;
-    const T Dmy = (c - ym) * inv, Dpy = (yp - c) * inv;
-    const T Dmz = (c - zm) * inv, Dpz = (zp - c) * inv;
-    const T amx = pos(Dmx), bmx = neg(Dmx), apx = pos(Dpx), bpx = neg(Dpx);
-    const T amy = pos(Dmy), bmy = neg(Dmy), apy = pos(Dpy), bpy = neg(Dpy);
-    const T amz = pos(Dmz), bmz = neg(Dmz), apz = pos(Dpz), bpz = neg(Dpz);
-    qp = ((amx * amx + bpx * bpx) + (amy * amy + bpy * bpy)) + (amz * amz + bpz * bpz);
-    qm = ((apx * apx + bmx * bmx) + (apy * apy + bmy * bmy)) + (apz * apz + bmz * bmz);
-}
-
-// eq. 7 (R5: test <= beta, then <= gamma, else 0)
-template <typename T>
-__device__ __forceinline__ T cutoff(T c, const StencilParams<T>& p) {
-    const T a = mag(c);
-    if (a <= p.beta) return T(1);
-    if (a <= p.gamma) {
-        const T t = a - p.gamma;
-        return ((t * t) * (((T(2) * a) + p.gamma) - p.three_beta)) * p.inv3;
-    }
-    return T(0);
-}
-
-// eq. 3 with eq. 8: phi - dt * (c(phi) * [max(F,0) grad+ + min(F,0) grad-]).
-template <typename T, bool DENSE>
-__device__ __forceinline__ T advance_value(T c, T xm, T xp, T ym, T yp, T zm, T zp, T f, const StencilParams<T>& p) {
-    T qp, qm;
-    upwind_q(c, xm, xp, ym, yp, zm, zp, p.inv_dx, qp, qm);
-    // f > 0: H = f*grad+ + 0*grad-;  f < 0: H = 0*grad+ + f*grad-;  f == 0: H = 0
-    const T H = f * root(f > T(0) ? qp : qm);
-    const T cf = DENSE ? T(1) : cutoff(c, p);
-    return c - p.dt * (cf * H);
-}
-
-// eq. 12-13 (R9-R12): d - dtau * [max(S,0)(grad+ - 1) + min(S,0)(grad- - 1)], S = d / sqrt(d^2 + |Dd|^2 dx^2),
-// |Dd|^2 = q+ if d > 0, q- if d < 0; S = 0 where the root vanishes.
-template <typename T>
-__device__ __forceinline__ T reinit_value(T c, T xm, T xp, T ym, T yp, T zm, T zp, const StencilParams<T>& p) {
-    T qp, qm;
-    upwind_q(c, xm, xp, ym, yp, zm, zp, p.inv_dx, qp, qm);
-    const T q = c > T(0) ? qp : (c < T(0) ? qm : T(0));
-    const T den = root(c * c + q * p.dx2);
-    const T S = den == T(0) ? T(0) : quot(c, den);
-    const T U = S * (root(q) - T(1));   // sign S = sign d picks the branch; the other term is an exact 0
-    return c - p.dt * U;
-}
-
-template <typename T>
-__device__ __forceinline__ T clamp_val(T v, T gamma) {
-    if (v < -gamma) v = -gamma;
-    if (v > gamma) v = gamma;
-    return v;
-}
 
 // Stage brick (x0,y0,z0) plus its six faces into s[z][y][x] (10^3, edges/corners skipped).
 // Indices are clamped to the domain: edge replicate (R3).
@@ -295,6 +230,12 @@ __global__ void __launch_bounds__(256) k_clamp_all_v4(float4* __restrict__ a, fl
 
 int band_grid() { return sm_count() * 8; }
 
+// Debug knob: LS_DISABLE_TMA=1 forces the scalar kernels (A/B timing, parity of the two paths).
+bool tma_disabled() {
+    static const bool off = [] { const char* e = getenv("LS_DISABLE_TMA"); return e && e[0] == '1'; }();
+    return off;
+}
+
 }  // namespace
 
 int sm_count() {
@@ -311,6 +252,9 @@ int sm_count() {
 template <typename T>
 void launch_advance_band(const T* phi, const T* F, T* out, const Geom& g, const StencilParams<T>& p,
                          const BandBuffers& bb, bool use_T_list, cudaStream_t s, int64_t* launches) {
+    if (!tma_disabled() && tma_usable<T>(g, phi, F, out) &&
+        launch_advance_tma<T>(phi, F, out, g, p, bb, use_T_list, s, launches))
+        return;
     if (use_T_list)
         k_advance_band<T><<<band_grid(), kBandThreads, 0, s>>>(phi, F, out, g, p, bb.T_ids, &bb.counts->nT, bb.T_masks,
                                                                nullptr, nullptr);
@@ -332,6 +276,9 @@ void launch_advance_dense(const T* phi, const T* F, T* out, const Geom& g, const
 template <typename T>
 void launch_reinit_band(const T* src, T* dst, const Geom& g, const StencilParams<T>& p, const BandBuffers& bb,
                         bool clamp, unsigned long long* residual, bool emit_T, cudaStream_t s, int64_t* launches) {
+    if (!tma_disabled() && tma_usable<T>(g, src, dst, nullptr) &&
+        launch_reinit_tma<T>(src, dst, g, p, bb, clamp, residual, emit_T, s, launches))
+        return;
     const int grid = band_grid();
     const int32_t* cnt = &bb.counts->nN;
 #define LS_LAUNCH(C, R, E)                                                                                        \
