@@ -26,7 +26,7 @@ KERNEL_KINDS = ("classify", "band", "advance", "reinit", "clamp", "copy")
 SYMBOLS = (
     "ls_status_str", "ls_last_cuda_error", "ls_create", "ls_destroy", "ls_build_band", "ls_band_counts",
     "ls_band_export", "ls_advance", "ls_reinit", "ls_reinit_tol", "ls_step", "ls_step_host", "ls_stats",
-    "ls_stats_reset", "ls_profile_enable", "ls_profile_read", "ls_profile_reset",
+    "ls_stats_reset", "ls_profile_enable", "ls_profile_read", "ls_profile_reset", "ls_selftest_math",
 )
 
 
@@ -76,6 +76,7 @@ def lib() -> C.CDLL:
         L.ls_profile_enable.argtypes = [_P, _I]
         L.ls_profile_read.argtypes = [_P, _I, C.POINTER(_D), C.POINTER(_L)]
         L.ls_profile_reset.argtypes = [_P]
+        L.ls_selftest_math.argtypes = [_P, C.c_uint64, _L, _D, _D, _D, _D, C.POINTER(_L)]
         for name in SYMBOLS[2:]:
             getattr(L, name).restype = C.c_int
         _lib = L
@@ -197,3 +198,11 @@ def ls_profile_read(ctx: int, kind: int):
 
 def ls_profile_reset(ctx: int) -> None:
     _ck(lib().ls_profile_reset(_P(ctx)), "ls_profile_reset")
+
+
+def ls_selftest_math(seed: int, n: int, dx: float, dt: float, beta: float, gamma: float, cuda_stream: int = 0) -> int:
+    """-> number of results (of 4n) where the packed fp32 pair arithmetic differs from the scalar IEEE path."""
+    m = _L()
+    _ck(lib().ls_selftest_math(_P(cuda_stream), C.c_uint64(seed), n, dx, dt, beta, gamma, C.byref(m)),
+        "ls_selftest_math")
+    return m.value

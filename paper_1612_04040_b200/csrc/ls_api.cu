@@ -251,7 +251,9 @@ ls_status ls_create(int32_t nx, int32_t ny, int32_t nz, ls_dtype dtype, void* cu
     ls_ctx* c = new (std::nothrow) ls_ctx();
     if (!c) return LS_ERR_ALLOC;
     std::memset(c, 0, sizeof *c);
-    c->g = ls::Geom{nx, ny, nz, (int)NBx, (int)NBy, (int)NBz, (int)nbricks};
+    auto bits = [](int64_t n) { int b = 0; while (((int64_t)1 << b) < n) ++b; return b; };   // ceil(log2 n)
+    const int wx = bits(NBx), wy = bits(NBy);   // wx + wy + bits(NBz) <= 27 + 3
+    c->g = ls::Geom{nx, ny, nz, (int)NBx, (int)NBy, (int)NBz, (int)nbricks, (1 << wx) - 1, (1 << wy) - 1, wx, wx + wy};
     c->dtype = dtype;
     c->stream = (cudaStream_t)cuda_stream;
     c->elem = dtype == LS_F32 ? 4 : 8;
@@ -277,6 +279,9 @@ ls_status ls_create(int32_t nx, int32_t ny, int32_t nz, ls_dtype dtype, void* cu
     alloc((void**)&bb.T_ids, (size_t)nbricks * 4, false);
     alloc((void**)&bb.N_ids, (size_t)nbricks * 4, false);
     alloc((void**)&bb.U_ids, (size_t)nbricks * 4, false);
+    alloc((void**)&bb.T_pos, (size_t)nbricks * 4, false);
+    alloc((void**)&bb.N_pos, (size_t)nbricks * 4, false);
+    alloc((void**)&bb.U_pos, (size_t)nbricks * 4, false);
     alloc((void**)&bb.T_masks, (size_t)nbricks * 64, false);
     alloc((void**)&bb.N_masks, (size_t)nbricks * 64, false);
     alloc((void**)&bb.partials, (size_t)bb.npartials * 3 * 4, true);
@@ -299,7 +304,7 @@ ls_status ls_destroy(ls_ctx* c) {
     if (!c) return LS_OK;
     cudaStreamSynchronize(c->stream);
     ls::BandBuffers& bb = c->bb;
-    void* dev[] = {bb.tmask, bb.nmask, bb.flagT, bb.flagN, bb.flagNprev, bb.T_ids, bb.N_ids, bb.U_ids,
+    void* dev[] = {bb.tmask, bb.nmask, bb.flagT, bb.flagN, bb.flagNprev, bb.T_ids, bb.N_ids, bb.U_ids, bb.T_pos, bb.N_pos, bb.U_pos,
                    bb.T_masks, bb.N_masks, bb.partials, bb.counts, c->residual, c->scratch, c->dev_phi, c->dev_F};
     for (void* p : dev)
         if (p) cudaFree(p);
@@ -529,6 +534,26 @@ ls_status ls_profile_reset(ls_ctx* c) {
     ls_status st = prof_collect(c);
     for (int k = 0; k < LS_K_KINDS; ++k) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
     return st;
+}
+
+ls_status ls_selftest_math(void* cuda_stream, uint64_t seed, int64_t n, double dx, double dt, double beta,
+                           double gamma, int64_t* mismatches) {
+    if (!mismatches || n < 0 || bad_band_params(dx, beta, gamma) || std::isinf(gamma)) return LS_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    unsigned long long* d = nullptr;
+    LS_CK(cudaMalloc((void**)&d, 8));
+    cudaError_t e = cudaMemsetAsync(d, 0, 8, s);
+    unsigned long long h = 0;
+    if (e == cudaSuccess) {
+        ls::launch_selftest_math(seed, n, make_params<float>(dx, dt, beta, gamma), d, s);
+        e = cudaPeekAtLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&h, d, 8, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    cudaFree(d);
+    if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(e, "ls_selftest_math"); }
+    *mismatches = (int64_t)h;
+    return LS_OK;
 }
 
 ls_status ls_stats_reset(ls_ctx* c) {

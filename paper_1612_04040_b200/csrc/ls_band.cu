@@ -244,7 +244,8 @@ __global__ void __launch_bounds__(kScanThreads) k_scatter(const uint8_t* __restr
                                                           const uint8_t* __restrict__ fP,
                                                           const int32_t* __restrict__ partials, int npartials,
                                                           const uint64_t* __restrict__ tmask,
-                                                          const uint64_t* __restrict__ nmask, BandBuffers bb) {
+                                                          const uint64_t* __restrict__ nmask, BandBuffers bb,
+                                                          Geom g) {
     __shared__ int wtot[3][kScanThreads / 32];
     const int base = blockIdx.x * kScanTile + threadIdx.x * kItemsPerThread;
     uint32_t m[3];
@@ -271,19 +272,24 @@ __global__ void __launch_bounds__(kScanThreads) k_scatter(const uint8_t* __restr
         excl[l] += off;
     }
     int ptsT = 0, ptsN = 0;
+    int bx = base % g.NBx, by = (base / g.NBx) % g.NBy, bz = base / (g.NBx * g.NBy);
     for (int i = 0; i < kItemsPerThread; ++i) {
         const int b = base + i;
+        const int pos = bx | (by << g.pos_sy) | (bz << g.pos_sz);
+        if (++bx == g.NBx) { bx = 0; if (++by == g.NBy) { by = 0; ++bz; } }
         if ((m[0] >> i) & 1u) {
             bb.T_ids[excl[0]] = b;
+            bb.T_pos[excl[0]] = pos;
             ptsT += copy_mask(tmask + (int64_t)b * 8, bb.T_masks + (int64_t)excl[0] * 8);
             ++excl[0];
         }
         if ((m[1] >> i) & 1u) {
             bb.N_ids[excl[1]] = b;
+            bb.N_pos[excl[1]] = pos;
             ptsN += copy_mask(nmask + (int64_t)b * 8, bb.N_masks + (int64_t)excl[1] * 8);
             ++excl[1];
         }
-        if ((m[2] >> i) & 1u) bb.U_ids[excl[2]++] = b;
+        if ((m[2] >> i) & 1u) { bb.U_ids[excl[2]] = b; bb.U_pos[excl[2]++] = pos; }
     }
     ptsT = warp_sum(ptsT);
     ptsN = warp_sum(ptsN);
@@ -321,7 +327,7 @@ void launch_dilate_compact(const Geom& g, const BandBuffers& bb, int iters, bool
     k_count<<<bb.npartials, kScanThreads, 0, s>>>(bb.flagT, bb.flagN, bb.flagNprev, bb.partials, bb.npartials);
     k_scan_partials<<<1, 1024, 0, s>>>(bb.partials, bb.npartials, bb.counts);
     k_scatter<<<bb.npartials, kScanThreads, 0, s>>>(bb.flagT, bb.flagN, bb.flagNprev, bb.partials, bb.npartials,
-                                                    bb.tmask, bb.nmask, bb);
+                                                    bb.tmask, bb.nmask, bb, g);
     k_finalize<<<1, 1, 0, s>>>(bb.counts, iters, count_step ? 1 : 0);
     if (launches) *launches += 5;
 }

@@ -11,6 +11,8 @@ struct Geom {
     int nx, ny, nz;
     int NBx, NBy, NBz;
     int nbricks;
+    // packed brick position of the list entries (T_pos / N_pos / U_pos): bx | by << pos_sy | bz << pos_sz
+    int pos_mx, pos_my, pos_sy, pos_sz;
     __host__ __device__ inline int64_t idx(int i, int j, int k) const {
         return ((int64_t)k * ny + j) * nx + i;
     }
@@ -40,6 +42,9 @@ struct BandBuffers {
     int32_t* N_ids;
     uint64_t* N_masks;
     int32_t* U_ids;
+    int32_t* T_pos;    // [nbricks] packed (bx, by, bz) of each list entry, see Geom::pos_*
+    int32_t* N_pos;
+    int32_t* U_pos;
     int32_t* partials; // [3 * npartials] per-CTA flag counts, then their exclusive scans
     int npartials;
     Counts* counts;
@@ -101,6 +106,10 @@ bool launch_reinit_tma(const T* src, T* dst, const Geom& g, const StencilParams<
 template <typename T>
 bool launch_advance_tma(const T* phi, const T* F, T* out, const Geom& g, const StencilParams<T>& p,
                         const BandBuffers& bb, bool use_T_list, cudaStream_t s, int64_t* launches);
+
+// Bit-for-bit check of the packed pair arithmetic against the scalar functions on n random stencil pairs.
+void launch_selftest_math(uint64_t seed, int64_t n, const StencilParams<float>& p, unsigned long long* mismatches,
+                          cudaStream_t s);
 
 int sm_count();
 

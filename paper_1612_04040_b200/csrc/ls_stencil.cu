@@ -228,6 +228,66 @@ __global__ void __launch_bounds__(256) k_clamp_all_v4(float4* __restrict__ a, fl
     }
 }
 
+// Device self-check of the packed two-point arithmetic (ls_math.cuh) against the scalar IEEE functions:
+// random 7-point stencils (smooth band-like values, wide-exponent values, exact zeros, flat patches),
+// both halves of a pair compared bit for bit.  Counts mismatching results.
+__device__ __forceinline__ uint64_t mix64(uint64_t z) {
+    z += 0x9E3779B97F4A7C15ull;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+__device__ __forceinline__ float test_value(uint64_t r, int kind, float centre) {
+    const float u = (float)(r >> 40) * (1.0f / 16777216.0f);   // [0, 1)
+    switch (kind) {
+        case 0: return centre + (u - 0.5f) * 0.004f;                         // smooth field, |grad| ~ 1 at dx = 1/512
+        case 1: return __uint_as_float((uint32_t)r & 0xff7fffffu);           // any finite-or-not bit pattern but NaN payloads kept rare
+        case 2: return 0.0f;
+        case 3: return centre;                                                // flat
+        default: return (u - 0.5f) * 0.03f;
+    }
+}
+__device__ __forceinline__ bool same_bits(float a, float b) {
+    return __float_as_uint(a) == __float_as_uint(b) || (a != a && b != b);
+}
+__global__ void __launch_bounds__(256) k_selftest_math(uint64_t seed, int64_t n, StencilParams<float> p,
+                                                       unsigned long long* mismatches) {
+    unsigned long long bad = 0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        // line[h][3 + d], d in {-3: zm, -2: ym, -1: xm, 0: c, 1: xp, 2: yp, 3: zp}: a "tile" with strides sy = 2, sz = 3
+        float line[16], f[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const uint64_t r = mix64(seed + (uint64_t)(2 * i + h) * 16);
+            const int mode = (int)(r & 7);
+            const float c = test_value(mix64(r), (mode == 7 || mode == 3) ? 1 : (mode == 6 ? 2 : 4), 0.f);
+#pragma unroll
+            for (int k = 0; k < 7; ++k) {
+                const uint64_t rk = mix64(r + 1 + k);
+                int kind = 0;
+                if (mode == 7) kind = 1;
+                else if (mode == 3) kind = 4;
+                else if (mode == 5) kind = (rk & 1) ? 3 : 0;
+                else if (mode == 4) kind = (rk & 3) == 0 ? 2 : 0;
+                line[8 * h + k] = k == 3 ? c : test_value(rk >> 2, kind, c);
+            }
+            line[8 * h + 7] = 0.f;
+            const uint64_t rf = mix64(r + 9);
+            f[h] = (rf & 15) == 0 ? 0.f : ((float)(rf >> 40) * (1.0f / 8388608.0f) - 1.0f);
+        }
+        const float* a = line;
+        const float* b = line + 8;
+        const float r0 = reinit_value<float>(a[3], a[2], a[4], a[1], a[5], a[0], a[6], p);
+        const float r1 = reinit_value<float>(b[3], b[2], b[4], b[1], b[5], b[0], b[6], p);
+        const float a0 = advance_value<float, false>(a[3], a[2], a[4], a[1], a[5], a[0], a[6], f[0], p);
+        const float a1 = advance_value<float, false>(b[3], b[2], b[4], b[1], b[5], b[0], b[6], f[1], p);
+        const Two<float> rp = reinit_pair<float>(line, 3, 11, 2, 3, p);
+        const Two<float> ap = advance_pair<float>(line, 3, 11, 2, 3, f[0], f[1], p);
+        bad += !same_bits(rp.x, r0) + !same_bits(rp.y, r1) + !same_bits(ap.x, a0) + !same_bits(ap.y, a1);
+    }
+    if (bad) atomicAdd(mismatches, bad);
+}
+
 int band_grid() { return sm_count() * 8; }
 
 // Debug knob: LS_DISABLE_TMA=1 forces the scalar kernels (A/B timing, parity of the two paths).
@@ -237,6 +297,11 @@ bool tma_disabled() {
 }
 
 }  // namespace
+
+void launch_selftest_math(uint64_t seed, int64_t n, const StencilParams<float>& p, unsigned long long* mismatches,
+                          cudaStream_t s) {
+    k_selftest_math<<<sm_count() * 8, 256, 0, s>>>(seed, n, p, mismatches);
+}
 
 int sm_count() {
     static int n = 0;

@@ -22,9 +22,11 @@ namespace ls {
 
 namespace {
 
-constexpr int kThreads = 256;
+constexpr int kThreads = 128;   // 4 warps: the per-brick bookkeeping every warp repeats is paid 4x, not 8x
 constexpr int kStages = 3;
 constexpr int kPY = 10;   // tile extent in y and z: 8 + one halo cell on each side
+constexpr int kListBytes = 512 * 4;
+constexpr int kBarBytes = 64;   // mbarriers
 
 template <typename T> struct TileCfg;
 // TMA needs every box row to start on a 16-byte boundary of the field and to span a multiple of 16
@@ -34,6 +36,15 @@ template <> struct TileCfg<float> { static constexpr int XOFF = 4, PX = 16; };
 template <> struct TileCfg<double> { static constexpr int XOFF = 2, PX = 12; };
 
 constexpr int round128(int x) { return (x + 127) / 128 * 128; }
+
+// Header of a stage, written by the producer thread before it starts the loads of the stage.
+struct alignas(16) Hdr {
+    int b;          // brick id
+    int x0, y0, z0; // first cell of the brick
+    long long org;  // element offset of that cell in the dense field
+    int edge;       // brick touches the domain boundary (halo needs patching, rows may be partial)
+    int has_T;      // Advance: the brick holds T points (mask and F were loaded)
+};
 
 // One pipeline stage in shared memory: [halo tile][F brick (Advance only)][mask 64 B][header 64 B].
 template <typename T, bool WITH_F>
@@ -48,17 +59,18 @@ struct Stage {
     static constexpr int OFF_HDR = OFF_MASK + 64;
     static constexpr int BYTES = OFF_HDR + 64;
     static_assert(BYTES % 128 == 0, "stages must keep 128-byte alignment");
+    static_assert(sizeof(Hdr) <= 64, "header slot");
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
@@ -67,47 +79,43 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "@p bra LS_DONE;\n"
         "bra LS_WAIT;\n"
         "LS_DONE:\n"
-        "}\n" ::"r"(smem_u32(bar)),
+        "}\n" ::"r"(bar),
         "r"(parity)
         : "memory");
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, uint64_t* bar, int x, int y, int z) {
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int x, int y, int z) {
     asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(
-            smem_u32(dst)),
-        "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(z)
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(dst),
+        "l"(map), "r"(bar), "r"(x), "r"(y), "r"(z)
         : "memory");
 }
-__device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
                  : "memory");
 }
 
-struct BrickPos {
-    int b, x0, y0, z0;
-};
-__device__ __forceinline__ BrickPos brick_pos(const Geom& g, int b) {
-    BrickPos q;
-    q.b = b;
-    const int bx = b % g.NBx, r = b / g.NBx;
-    q.x0 = bx * 8;
-    q.y0 = (r % g.NBy) * 8;
-    q.z0 = (r / g.NBy) * 8;
-    return q;
+// Producer side: decode the packed brick position (Geom::pos_*), fill the header.
+__device__ __forceinline__ void fill_hdr(Hdr* h, const Geom& g, int b, int pos, bool has_T) {
+    const int bx = pos & g.pos_mx, by = (pos >> g.pos_sy) & g.pos_my, bz = pos >> g.pos_sz;
+    h->b = b;
+    h->x0 = bx * 8;
+    h->y0 = by * 8;
+    h->z0 = bz * 8;
+    h->org = g.idx(bx * 8, by * 8, bz * 8);
+    h->edge = (bx == 0) | (by == 0) | (bz == 0) | (bx == g.NBx - 1) | (by == g.NBy - 1) | (bz == g.NBz - 1);
+    h->has_T = has_T ? 1 : 0;
 }
 
 // R3: TMA zero-fills cells outside the domain; give them the value of the nearest in-domain cell
 // (edge replicate).  Sources are in-domain cells, destinations are not: no ordering needed inside.
+// Only called for bricks on the domain boundary (block-uniform).
 template <typename T, int PX, int XOFF>
-__device__ __forceinline__ void patch_boundary(T* tile, const Geom& g, const BrickPos& q) {
-    const bool edge = q.x0 == 0 || q.y0 == 0 || q.z0 == 0 || q.x0 + 8 >= g.nx || q.y0 + 8 >= g.ny || q.z0 + 8 >= g.nz;
-    if (!edge) return;   // uniform over the CTA
-    const int ox = q.x0 - XOFF, oy = q.y0 - 1, oz = q.z0 - 1;
+__device__ __noinline__ void patch_boundary(T* tile, const Geom& g, int x0, int y0, int z0) {
+    const int ox = x0 - XOFF, oy = y0 - 1, oz = z0 - 1;
     for (int e = threadIdx.x; e < PX * kPY * kPY; e += kThreads) {
         const int x = e % PX, r = e / PX, y = r % kPY, z = r / kPY;
         const int gx = ox + x, gy = oy + y, gz = oz + z;
@@ -117,149 +125,185 @@ __device__ __forceinline__ void patch_boundary(T* tile, const Geom& g, const Bri
             if (sx >= 0 && sx < PX && sy < kPY && sz < kPY) tile[e] = tile[(sz * kPY + sy) * PX + sx];
         }
     }
+    fence_proxy_async();   // generic writes into a tile a later TMA load overwrites
     __syncthreads();
 }
 
-// Compact the set bits of the brick mask into `list` (tile offsets of the active points, ascending
-// point order) and return their number.  Warp w owns mask word w (layer lz = w): lane l holds bit l of
-// the low half (row l>>3) and of the high half (row 4 + (l>>3)).
+// Compact the set bits of the brick mask into `list` (ascending point order) and return their number.
+// Entry = tile offset of the point | brick-local index (lz*64 + ly*8 + lx) << 16.
+// Warp w owns mask words 2w and 2w+1 (layers lz): lane l holds bit l of the low half (row l>>3) and
+// of the high half (row 4 + (l>>3)) of each.
 template <int PX, int XOFF>
-__device__ __forceinline__ int build_list(const uint64_t* mk, uint16_t* list, uint32_t& lo, uint32_t& hi, int& off_lo) {
+__device__ __forceinline__ int build_list(const uint64_t* mk, uint32_t* list) {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const uint64_t word = mk[w];
-    lo = (uint32_t)word;
-    hi = (uint32_t)(word >> 32);
-    const int pc = lane < 8 ? __popcll(mk[lane]) : 0;
-    int incl = pc;
-#pragma unroll
-    for (int o = 1; o < 8; o <<= 1) {
-        const int y = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += y;
-    }
-    const int total = __shfl_sync(0xffffffffu, incl, 7);
-    const int base = __shfl_sync(0xffffffffu, incl - pc, w);
+    const unsigned pc = lane < 8 ? __popcll(mk[lane]) : 0;
+    const int total = (int)__reduce_add_sync(0xffffffffu, pc);
+    int base = (int)__reduce_add_sync(0xffffffffu, lane < 2 * w ? pc : 0u);   // points in layers below 2w
+    const ulonglong2 words = *reinterpret_cast<const ulonglong2*>(mk + 2 * w);
     const uint32_t lt = (1u << lane) - 1u;
-    off_lo = ((w + 1) * kPY + (lane >> 3) + 1) * PX + (lane & 7) + XOFF;
-    if ((lo >> lane) & 1u) list[base + __popc(lo & lt)] = (uint16_t)off_lo;
-    if ((hi >> lane) & 1u) list[base + __popc(lo) + __popc(hi & lt)] = (uint16_t)(off_lo + 4 * PX);
+    const uint32_t e0 = (uint32_t)((2 * w + 1) * kPY * PX + ((lane >> 3) + 1) * PX + (lane & 7) + XOFF) |
+                        (uint32_t)(2 * w * 64 + lane) << 16;   // layer 2w, low half (rows 0-3)
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const uint64_t word = h ? words.y : words.x;
+        const uint32_t lo = (uint32_t)word, hi = (uint32_t)(word >> 32);
+        const uint32_t e_lo = e0 + h * (uint32_t)(kPY * PX + (64 << 16));
+        const int nlo = __popc(lo);
+        if ((lo >> lane) & 1u) list[base + __popc(lo & lt)] = e_lo;
+        if ((hi >> lane) & 1u) list[base + nlo + __popc(hi & lt)] = e_lo + (uint32_t)(4 * PX + (32 << 16));
+        base += nlo + __popc(hi);
+    }
     return total;
 }
 
-// Store rows of the brick from the tile to dst with 128-bit stores.  A row (8 cells, 32 B in fp32)
-// is written if `all_rows` or it holds a mask bit, and lies inside the domain.
+// Per-thread constants of the row store: thread t owns 128-bit part `part` of brick row `row`
+// (fp32: 64 rows x 2 parts = 128 threads, one pass; fp64: 64 rows x 4 parts, two passes).
+template <typename T>
+struct RowSlot {
+    int row;        // lz*8 + ly
+    int toff;       // tile offset of the first cell of the part
+    long long goff; // element offset from the brick origin
+    int lx0, ly, lz;
+};
 template <typename T, int PX, int XOFF>
-__device__ __forceinline__ void store_rows(const T* tile, const uint64_t* mk, bool all_rows, T* __restrict__ dst,
-                                           const Geom& g, const BrickPos& q) {
-    constexpr int VEC = 16 / (int)sizeof(T);   // cells per 128-bit store
-    constexpr int PARTS = 8 / VEC;             // stores per row
-    const int t = threadIdx.x;
-    if (t >= 64 * PARTS) return;
-    const int row = t / PARTS, part = t % PARTS;
-    const int lz = row >> 3, ly = row & 7;
-    const bool want = all_rows || ((mk[lz] >> (8 * ly)) & 0xffull) != 0;
-    const int i = q.x0 + part * VEC, j = q.y0 + ly, k = q.z0 + lz;
-    if (!want || i >= g.nx || j >= g.ny || k >= g.nz) return;   // nx % VEC == 0: a part is all in or all out
-    const T* s = tile + ((lz + 1) * kPY + (ly + 1)) * PX + XOFF + part * VEC;
-    T* d = dst + g.idx(i, j, k);
-    *reinterpret_cast<int4*>(d) = *reinterpret_cast<const int4*>(s);   // XOFF*sizeof(T) == 16: aligned
+__device__ __forceinline__ RowSlot<T> row_slot(const Geom& g, int t) {
+    constexpr int VEC = 16 / (int)sizeof(T), PARTS = 8 / VEC;
+    RowSlot<T> r;
+    r.row = t / PARTS;
+    const int part = t % PARTS;
+    r.lz = r.row >> 3;
+    r.ly = r.row & 7;
+    r.lx0 = part * VEC;
+    r.toff = ((r.lz + 1) * kPY + (r.ly + 1)) * PX + XOFF + part * VEC;
+    r.goff = ((long long)r.lz * g.ny + r.ly) * g.nx + part * VEC;
+    return r;
+}
+// Store the part: new values (out brick, indexed by brick-local cell) where the mask bit is set, the
+// tile's values elsewhere.  Rows without a mask bit are skipped unless all_rows (then copied from the tile).
+template <typename T>
+__device__ __forceinline__ void store_part(const T* tile, const T* outb, const unsigned char* mk8, bool have_mask,
+                                           bool all_rows, T* __restrict__ dst, const Geom& g, const Hdr& h,
+                                           const RowSlot<T>& r) {
+    constexpr int VEC = 16 / (int)sizeof(T);
+    const unsigned m = have_mask ? mk8[r.row] : 0u;
+    if (!all_rows && m == 0) return;
+    if (h.edge && (h.x0 + r.lx0 >= g.nx || h.y0 + r.ly >= g.ny || h.z0 + r.lz >= g.nz)) return;   // nx % VEC == 0
+    union V { int4 q; T e[VEC]; } a, b;
+    a.q = *reinterpret_cast<const int4*>(tile + r.toff);
+    const unsigned nib = (m >> r.lx0) & ((1u << VEC) - 1u);
+    if (nib) {
+        b.q = *reinterpret_cast<const int4*>(outb + r.row * 8 + r.lx0);
+#pragma unroll
+        for (int e = 0; e < VEC; ++e)
+            if ((nib >> e) & 1u) a.e[e] = b.e[e];
+    }
+    *reinterpret_cast<int4*>(dst + h.org + r.goff) = a.q;
 }
 
 // ---------------------------------------------------------------------------------------------
 // Step 3: one reinitialisation sweep over the N list (eq. 12-13), see launch_reinit_band.
 // ---------------------------------------------------------------------------------------------
 template <typename T, bool CLAMP, bool RESIDUAL, bool EMIT_T>
-__global__ void __launch_bounds__(kThreads, 6)
+__global__ void __launch_bounds__(kThreads)
 k_reinit_tma(const __grid_constant__ CUtensorMap tm_src, T* __restrict__ dst, Geom g, StencilParams<T> p,
-             const int32_t* __restrict__ ids, const int32_t* __restrict__ count_ptr,
+             const int32_t* __restrict__ ids, const int32_t* __restrict__ poss, const int32_t* __restrict__ count_ptr,
              const uint64_t* __restrict__ masks, unsigned long long* __restrict__ residual,
              uint64_t* __restrict__ tmask, uint8_t* __restrict__ flagT) {
     using S = Stage<T, false>;
     constexpr int PX = S::PX, XOFF = S::XOFF;
+    constexpr int SY = PX, SZ = kPY * PX;
+    constexpr int PASSES = (64 * (8 / (16 / (int)sizeof(T)))) / kThreads;   // row-store passes: 1 (fp32), 2 (fp64)
+    // dynamic shared memory: [kStages stages][list 2 KB][out brick 8^3][mbarriers] — one base register for all
     extern __shared__ __align__(128) unsigned char smem[];
-    __shared__ uint64_t full[kStages];
-    __shared__ uint16_t list[512];
+    uint32_t* list = reinterpret_cast<uint32_t*>(smem + kStages * S::BYTES);
+    T* outb = reinterpret_cast<T*>(smem + kStages * S::BYTES + kListBytes);
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int count = *count_ptr;
     const int G = gridDim.x;
     const int mine = (int)blockIdx.x < count ? (count - (int)blockIdx.x + G - 1) / G : 0;
+    const uint32_t smem_base = smem_u32(smem), bar_base = smem_base + kStages * S::BYTES + kListBytes + 512 * (int)sizeof(T);
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
+        for (int s = 0; s < kStages; ++s) mbar_init(bar_base + 8 * s, 1);
         fence_barrier_init();
     }
     __syncthreads();
 
-    auto issue = [&](int n, int b) {   // thread 0: start the loads of my n-th brick (list index li, id b)
-        const int li = blockIdx.x + n * G;
-        unsigned char* st = smem + (n % kStages) * S::BYTES;
-        uint64_t* bar = &full[n % kStages];
-        const BrickPos q = brick_pos(g, b);
-        *reinterpret_cast<int*>(st + S::OFF_HDR) = b;
+    RowSlot<T> rs[PASSES];
+#pragma unroll
+    for (int q = 0; q < PASSES; ++q) rs[q] = row_slot<T, PX, XOFF>(g, tid + q * kThreads);
+
+    // producer state (thread 0): next list index to issue and the stage it goes to
+    int p_li = blockIdx.x, p_slot = 0, p_left = mine;
+    auto issue = [&]() {
+        const int b = ids[p_li], pos = poss[p_li];
+        Hdr* h = reinterpret_cast<Hdr*>(smem + p_slot * S::BYTES + S::OFF_HDR);
+        fill_hdr(h, g, b, pos, true);
+        if (EMIT_T) flagT[b] = 0;
+        const uint32_t st = smem_base + p_slot * S::BYTES, bar = bar_base + 8 * p_slot;
         mbar_expect_tx(bar, S::TILE_BYTES + 64);
-        tma_load_3d(st, &tm_src, bar, q.x0 - XOFF, q.y0 - 1, q.z0 - 1);
-        bulk_load(st + S::OFF_MASK, masks + (int64_t)li * 8, 64, bar);
+        tma_load_3d(st, &tm_src, bar, h->x0 - XOFF, h->y0 - 1, h->z0 - 1);
+        bulk_load(st + S::OFF_MASK, masks + (int64_t)p_li * 8, 64, bar);
+        p_li += G;
+        p_slot = p_slot == kStages - 1 ? 0 : p_slot + 1;
+        --p_left;
     };
-    int b_next = 0;   // id of my brick number (n + kStages - 1), prefetched one iteration ahead
-    if (tid == 0) {
-        for (int n = 0; n < kStages - 1 && n < mine; ++n) issue(n, ids[blockIdx.x + n * G]);
-        if (kStages - 1 < mine) b_next = ids[blockIdx.x + (kStages - 1) * G];
-    }
+    if (tid == 0)
+        for (int n = 0; n < kStages - 1 && p_left > 0; ++n) issue();
 
     T rmax = T(0);
+    int slot = 0;
+    uint32_t phase = 0;
     for (int n = 0; n < mine; ++n) {
-        if (tid == 0 && n + kStages - 1 < mine) {
-            issue(n + kStages - 1, b_next);
-            if (n + kStages < mine) b_next = ids[blockIdx.x + (n + kStages) * G];
-        }
-        unsigned char* st = smem + (n % kStages) * S::BYTES;
-        T* tile = reinterpret_cast<T*>(st);
+        unsigned char* st = smem + slot * S::BYTES;
+        const T* tile = reinterpret_cast<const T*>(st);
         const uint64_t* mk = reinterpret_cast<const uint64_t*>(st + S::OFF_MASK);
-        mbar_wait(&full[n % kStages], (uint32_t)((n / kStages) & 1));
-        const BrickPos q = brick_pos(g, *reinterpret_cast<const int*>(st + S::OFF_HDR));
-        patch_boundary<T, PX, XOFF>(tile, g, q);
+        mbar_wait(bar_base + 8 * slot, phase);
+        const Hdr h = *reinterpret_cast<const Hdr*>(st + S::OFF_HDR);
+        if (h.edge) patch_boundary<T, PX, XOFF>(reinterpret_cast<T*>(st), g, h.x0, h.y0, h.z0);
 
-        uint32_t lo, hi;
-        int off_lo;
-        const int total = build_list<PX, XOFF>(mk, list, lo, hi, off_lo);
-        __syncthreads();
+        const int total = build_list<PX, XOFF>(mk, list);
+        __syncthreads();   // B1: list complete; every thread is done with brick n-1 (its stage, list, out brick)
+        if (tid == 0 && p_left > 0) issue();   // refill the stage brick n-1 used
 
-        T v[2];
-        int off[2];
+        // two points per thread and round; at most 512 points = 2 rounds of 128 pairs.  Jacobi: reads come
+        // from the tile (iteration k), results go to the out brick (iteration k+1).
 #pragma unroll
         for (int r = 0; r < 2; ++r) {
-            const int e = tid + r * kThreads;
-            off[r] = -1;
+            const int e = 2 * (tid + r * kThreads);
             if (e < total) {
-                const int o = list[e];
-                off[r] = o;
-                const T c = tile[o];
-                T u = reinit_value<T>(c, tile[o - 1], tile[o + 1], tile[o - PX], tile[o + PX], tile[o - kPY * PX],
-                                      tile[o + kPY * PX], p);
-                if (RESIDUAL) rmax = fmax(rmax, mag(u - c));
-                if (CLAMP) u = clamp_val(u, p.gamma);
-                v[r] = u;
+                uint2 ent = *reinterpret_cast<const uint2*>(list + e);
+                if (e + 1 >= total) ent.y = ent.x;   // odd tail: evaluate the last point twice
+                const int o0 = (int)(ent.x & 0xffffu), o1 = (int)(ent.y & 0xffffu);
+                Two<T> u = reinit_pair<T>(tile, o0, o1, SY, SZ, p);
+                if (RESIDUAL) rmax = fmax(rmax, fmax(mag(u.x - tile[o0]), mag(u.y - tile[o1])));
+                if (CLAMP) { u.x = clamp_val(u.x, p.gamma); u.y = clamp_val(u.y, p.gamma); }
+                outb[ent.x >> 16] = u.x;
+                outb[ent.y >> 16] = u.y;
             }
         }
-        __syncthreads();   // every neighbour read of iteration k is done: write iteration k+1 in place
-#pragma unroll
-        for (int r = 0; r < 2; ++r)
-            if (off[r] >= 0) tile[off[r]] = v[r];
-        fence_proxy_async();   // the next TMA load into this stage must order after these generic writes
-        __syncthreads();
+        __syncthreads();   // B2: out brick complete
 
-        store_rows<T, PX, XOFF>(tile, mk, false, dst, g, q);
+#pragma unroll
+        for (int q = 0; q < PASSES; ++q)
+            store_part<T>(tile, outb, reinterpret_cast<const unsigned char*>(mk), true, false, dst, g, h, rs[q]);
         if (EMIT_T) {
             // T mask of phi^{n+1} = clamp(d) on this brick: T^{n+1} is a subset of N^n
-            const bool tl = ((lo >> lane) & 1u) && mag(tile[off_lo]) < p.gamma;
-            const bool th = ((hi >> lane) & 1u) && mag(tile[off_lo + 4 * PX]) < p.gamma;
-            const uint32_t bl = __ballot_sync(0xffffffffu, tl), bh = __ballot_sync(0xffffffffu, th);
-            const uint64_t word = (uint64_t)bl | ((uint64_t)bh << 32);
-            if (lane == 0) tmask[(int64_t)q.b * 8 + w] = word;
-            const int any = __syncthreads_or(word != 0);
-            if (tid == 0) flagT[q.b] = any ? 1 : 0;
-        } else {
-            __syncthreads();   // stage is free for the producer
+            bool any = false;
+#pragma unroll
+            for (int hh = 0; hh < 2; ++hh) {
+                const int lz = 2 * w + hh;
+                const uint64_t word = mk[lz];
+                const bool tl = ((uint32_t)word >> lane) & 1u ? mag(outb[lz * 64 + lane]) < p.gamma : false;
+                const bool th = ((uint32_t)(word >> 32) >> lane) & 1u ? mag(outb[lz * 64 + 32 + lane]) < p.gamma : false;
+                const uint32_t bl = __ballot_sync(0xffffffffu, tl), bh = __ballot_sync(0xffffffffu, th);
+                const uint64_t tw = (uint64_t)bl | ((uint64_t)bh << 32);
+                if (lane == 0) tmask[(int64_t)h.b * 8 + lz] = tw;
+                any = any || tw != 0;
+            }
+            if (lane == 0 && any) flagT[h.b] = 1;   // zeroed by the producer when it issued the brick (barriers in between)
         }
+        if (++slot == kStages) { slot = 0; phase ^= 1u; }
     }
     if (RESIDUAL) {
         // non-negative IEEE values order like their bit patterns
@@ -281,108 +325,98 @@ k_reinit_tma(const __grid_constant__ CUtensorMap tm_src, T* __restrict__ dst, Ge
 //   dense_tmask == null: T list with its list-ordered masks
 // ---------------------------------------------------------------------------------------------
 template <typename T>
-__global__ void __launch_bounds__(kThreads, 5)
+__global__ void __launch_bounds__(kThreads)
 k_advance_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUtensorMap tm_F,
               T* __restrict__ out, Geom g, StencilParams<T> p, const int32_t* __restrict__ ids,
-              const int32_t* __restrict__ count_ptr, const uint64_t* __restrict__ list_masks,
-              const uint64_t* __restrict__ dense_tmask, const uint8_t* __restrict__ flagT) {
+              const int32_t* __restrict__ poss, const int32_t* __restrict__ count_ptr,
+              const uint64_t* __restrict__ list_masks, const uint64_t* __restrict__ dense_tmask,
+              const uint8_t* __restrict__ flagT) {
     using S = Stage<T, true>;
     constexpr int PX = S::PX, XOFF = S::XOFF;
+    constexpr int SY = PX, SZ = kPY * PX;
+    constexpr int PASSES = (64 * (8 / (16 / (int)sizeof(T)))) / kThreads;
+    // dynamic shared memory: [kStages stages][list 2 KB][out brick 8^3][mbarriers] — one base register for all
     extern __shared__ __align__(128) unsigned char smem[];
-    __shared__ uint64_t full[kStages];
-    __shared__ uint16_t list[512];
+    uint32_t* list = reinterpret_cast<uint32_t*>(smem + kStages * S::BYTES);
+    T* outb = reinterpret_cast<T*>(smem + kStages * S::BYTES + kListBytes);
     const int tid = threadIdx.x;
     const int count = *count_ptr;
     const int G = gridDim.x;
     const int mine = (int)blockIdx.x < count ? (count - (int)blockIdx.x + G - 1) / G : 0;
+    const uint32_t smem_base = smem_u32(smem), bar_base = smem_base + kStages * S::BYTES + kListBytes + 512 * (int)sizeof(T);
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
+        for (int s = 0; s < kStages; ++s) mbar_init(bar_base + 8 * s, 1);
         fence_barrier_init();
     }
     __syncthreads();
 
-    auto issue = [&](int n, int b, bool has_T) {
-        const int li = blockIdx.x + n * G;
-        unsigned char* st = smem + (n % kStages) * S::BYTES;
-        uint64_t* bar = &full[n % kStages];
-        const BrickPos q = brick_pos(g, b);
-        int* hdr = reinterpret_cast<int*>(st + S::OFF_HDR);
-        hdr[0] = b;
-        hdr[1] = has_T ? 1 : 0;
+    RowSlot<T> rs[PASSES];
+#pragma unroll
+    for (int q = 0; q < PASSES; ++q) rs[q] = row_slot<T, PX, XOFF>(g, tid + q * kThreads);
+
+    int p_li = blockIdx.x, p_slot = 0, p_left = mine;
+    auto issue = [&]() {
+        const int b = ids[p_li], pos = poss[p_li];
+        const bool has_T = dense_tmask ? flagT[b] != 0 : true;
+        Hdr* h = reinterpret_cast<Hdr*>(smem + p_slot * S::BYTES + S::OFF_HDR);
+        fill_hdr(h, g, b, pos, has_T);
+        const uint32_t st = smem_base + p_slot * S::BYTES, bar = bar_base + 8 * p_slot;
         mbar_expect_tx(bar, has_T ? S::TILE_BYTES + S::F_BYTES + 64 : S::TILE_BYTES);
-        tma_load_3d(st, &tm_phi, bar, q.x0 - XOFF, q.y0 - 1, q.z0 - 1);
+        tma_load_3d(st, &tm_phi, bar, h->x0 - XOFF, h->y0 - 1, h->z0 - 1);
         if (has_T) {
-            tma_load_3d(st + S::OFF_F, &tm_F, bar, q.x0, q.y0, q.z0);
-            const uint64_t* m = dense_tmask ? dense_tmask + (int64_t)b * 8 : list_masks + (int64_t)li * 8;
+            tma_load_3d(st + S::OFF_F, &tm_F, bar, h->x0, h->y0, h->z0);
+            const uint64_t* m = dense_tmask ? dense_tmask + (int64_t)b * 8 : list_masks + (int64_t)p_li * 8;
             bulk_load(st + S::OFF_MASK, m, 64, bar);
         }
+        p_li += G;
+        p_slot = p_slot == kStages - 1 ? 0 : p_slot + 1;
+        --p_left;
     };
-    auto fetch = [&](int n, int& b, bool& has_T) {
-        b = ids[blockIdx.x + n * G];
-        has_T = dense_tmask ? flagT[b] != 0 : true;
-    };
-    int b_next = 0;
-    bool t_next = false;
-    if (tid == 0) {
-        for (int n = 0; n < kStages - 1 && n < mine; ++n) {
-            int b;
-            bool h;
-            fetch(n, b, h);
-            issue(n, b, h);
-        }
-        if (kStages - 1 < mine) fetch(kStages - 1, b_next, t_next);
-    }
+    if (tid == 0)
+        for (int n = 0; n < kStages - 1 && p_left > 0; ++n) issue();
 
+    int slot = 0;
+    uint32_t phase = 0;
     for (int n = 0; n < mine; ++n) {
-        if (tid == 0 && n + kStages - 1 < mine) {
-            issue(n + kStages - 1, b_next, t_next);
-            if (n + kStages < mine) fetch(n + kStages, b_next, t_next);
-        }
-        unsigned char* st = smem + (n % kStages) * S::BYTES;
-        T* tile = reinterpret_cast<T*>(st);
+        unsigned char* st = smem + slot * S::BYTES;
+        const T* tile = reinterpret_cast<const T*>(st);
         const T* Fb = reinterpret_cast<const T*>(st + S::OFF_F);
         const uint64_t* mk = reinterpret_cast<const uint64_t*>(st + S::OFF_MASK);
-        mbar_wait(&full[n % kStages], (uint32_t)((n / kStages) & 1));
-        const int* hdr = reinterpret_cast<const int*>(st + S::OFF_HDR);
-        const BrickPos q = brick_pos(g, hdr[0]);
-        const bool has_T = hdr[1] != 0;
-        patch_boundary<T, PX, XOFF>(tile, g, q);
+        mbar_wait(bar_base + 8 * slot, phase);
+        const Hdr h = *reinterpret_cast<const Hdr*>(st + S::OFF_HDR);
+        if (h.edge) patch_boundary<T, PX, XOFF>(reinterpret_cast<T*>(st), g, h.x0, h.y0, h.z0);
 
-        if (has_T) {   // uniform over the CTA
-            uint32_t lo, hi;
-            int off_lo;
-            const int total = build_list<PX, XOFF>(mk, list, lo, hi, off_lo);
-            __syncthreads();
-            T v[2];
-            int off[2];
+        int total = 0;
+        if (h.has_T) total = build_list<PX, XOFF>(mk, list);   // uniform over the CTA
+        __syncthreads();   // B1: list complete; every thread is done with brick n-1
+        if (tid == 0 && p_left > 0) issue();
 #pragma unroll
-            for (int r = 0; r < 2; ++r) {
-                const int e = tid + r * kThreads;
-                off[r] = -1;
-                if (e < total) {
-                    const int o = list[e];
-                    off[r] = o;
-                    // tile offset -> brick-local (lx, ly, lz) -> index into the dense 8^3 F box
-                    const int x = o % PX - XOFF, rr = o / PX, y = rr % kPY - 1, z = rr / kPY - 1;
-                    const T f = Fb[(z * 8 + y) * 8 + x];
-                    v[r] = advance_value<T, false>(tile[o], tile[o - 1], tile[o + 1], tile[o - PX], tile[o + PX],
-                                                   tile[o - kPY * PX], tile[o + kPY * PX], f, p);
-                }
+        for (int r = 0; r < 2; ++r) {
+            const int e = 2 * (tid + r * kThreads);
+            if (e < total) {
+                uint2 ent = *reinterpret_cast<const uint2*>(list + e);
+                if (e + 1 >= total) ent.y = ent.x;
+                const Two<T> u = advance_pair<T>(tile, (int)(ent.x & 0xffffu), (int)(ent.y & 0xffffu), SY, SZ,
+                                                 Fb[ent.x >> 16], Fb[ent.y >> 16], p);
+                outb[ent.x >> 16] = u.x;
+                outb[ent.y >> 16] = u.y;
             }
-            __syncthreads();
-#pragma unroll
-            for (int r = 0; r < 2; ++r)
-                if (off[r] >= 0) tile[off[r]] = v[r];
-            fence_proxy_async();
-            __syncthreads();
         }
-        store_rows<T, PX, XOFF>(tile, mk, true, out, g, q);
-        __syncthreads();
+        __syncthreads();   // B2: out brick complete
+#pragma unroll
+        for (int q = 0; q < PASSES; ++q)
+            store_part<T>(tile, outb, reinterpret_cast<const unsigned char*>(mk), h.has_T != 0, true, out, g, h, rs[q]);
+        if (++slot == kStages) { slot = 0; phase ^= 1u; }
     }
 }
 
 int tma_grid(int ctas_per_sm) { return sm_count() * ctas_per_sm; }
+// Resident CTAs per SM by shared memory: 227 KB usable, 1 KB reserved per CTA, ~3 KB static (list, barriers).
+int ctas_per_sm(size_t dyn_smem) {
+    const int n = (int)((227 * 1024) / (dyn_smem + 4 * 1024));
+    return n < 1 ? 1 : (n > 12 ? 12 : n);
+}
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -440,15 +474,15 @@ bool launch_reinit_tma(const T* src, T* dst, const Geom& g, const StencilParams<
     using S = Stage<T, false>;
     CUtensorMap tm;
     if (!make_map<T>(&tm, src, g, S::PX, kPY, kPY)) return false;
-    const int grid = tma_grid(6);
-    const size_t shm = (size_t)kStages * S::BYTES;
+    const size_t shm = (size_t)kStages * S::BYTES + kListBytes + 512 * sizeof(T) + kBarBytes;
+    const int grid = tma_grid(ctas_per_sm(shm));
     const int32_t* cnt = &bb.counts->nN;
 #define LS_LAUNCH(C, R, E)                                                                                       \
     do {                                                                                                         \
         static bool once = (prefer_smem(k_reinit_tma<T, C, R, E>), true);                                        \
         (void)once;                                                                                              \
-        k_reinit_tma<T, C, R, E><<<grid, kThreads, shm, s>>>(tm, dst, g, p, bb.N_ids, cnt, bb.N_masks, residual, \
-                                                             bb.tmask, bb.flagT);                                \
+        k_reinit_tma<T, C, R, E><<<grid, kThreads, shm, s>>>(tm, dst, g, p, bb.N_ids, bb.N_pos, cnt, bb.N_masks,    \
+                                                             residual, bb.tmask, bb.flagT);                      \
     } while (0)
     if (emit_T) LS_LAUNCH(true, false, true);
     else if (residual && clamp) LS_LAUNCH(true, true, false);
@@ -468,14 +502,14 @@ bool launch_advance_tma(const T* phi, const T* F, T* out, const Geom& g, const S
     if (!make_map<T>(&tm_phi, phi, g, S::PX, kPY, kPY) || !make_map<T>(&tm_F, F, g, 8, 8, 8)) return false;
     static bool once = (prefer_smem(k_advance_tma<T>), true);
     (void)once;
-    const int grid = tma_grid(5);
-    const size_t shm = (size_t)kStages * S::BYTES;
+    const size_t shm = (size_t)kStages * S::BYTES + kListBytes + 512 * sizeof(T) + kBarBytes;
+    const int grid = tma_grid(ctas_per_sm(shm));
     if (use_T_list)
-        k_advance_tma<T><<<grid, kThreads, shm, s>>>(tm_phi, tm_F, out, g, p, bb.T_ids, &bb.counts->nT, bb.T_masks,
-                                                     nullptr, nullptr);
+        k_advance_tma<T><<<grid, kThreads, shm, s>>>(tm_phi, tm_F, out, g, p, bb.T_ids, bb.T_pos, &bb.counts->nT,
+                                                     bb.T_masks, nullptr, nullptr);
     else
-        k_advance_tma<T><<<grid, kThreads, shm, s>>>(tm_phi, tm_F, out, g, p, bb.U_ids, &bb.counts->nU, nullptr,
-                                                     bb.tmask, bb.flagT);
+        k_advance_tma<T><<<grid, kThreads, shm, s>>>(tm_phi, tm_F, out, g, p, bb.U_ids, bb.U_pos, &bb.counts->nU,
+                                                     nullptr, bb.tmask, bb.flagT);
     if (launches) *launches += 1;
     return true;
 }

@@ -80,3 +80,41 @@ def test_product_does_not_import_oracle():
         text = path.read_text()
         assert "import oracle" not in text and "from oracle" not in text and "ls_oracle" not in text, path
         assert "liboracle" not in text, path
+
+
+def test_packed_fp32_arithmetic_is_not_contracted():
+    """The fp32 band kernels use packed FMUL2 / FADD2 / FFMA2.  ptxas 12.9 contracts mul.rn.f32x2 +
+    add.rn.f32x2 into FFMA2 even under -fmad=false, which would break the arithmetic contract (R18: no
+    FMA contraction); ls_math.cuh routes every sum of a product through scalar adds to prevent it.
+    The only FFMA2 left are the explicit ones of the correctly rounded sqrt (2 per pair) and divide (5 per
+    pair) sequences: 2 evaluation rounds x (2 sqrt + 1 div) = 18 in a reinit kernel, 2 x 1 sqrt = 4 in
+    Advance.  A different count means the toolchain fused (or split) something: fail here, on the CPU."""
+    import re
+    import shutil
+    import subprocess
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not Path(cuobjdump).exists():
+        pytest.skip("cuobjdump not available")
+    from paper_1612_04040_b200 import build as ls_build
+    so = ls_build.build()
+    sass = subprocess.run([cuobjdump, "-sass", str(so)], capture_output=True, text=True, check=True).stdout
+    counts, tma_ops = {}, {}
+    fn = None
+    for line in sass.splitlines():
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            fn = m.group(1)
+            continue
+        if fn and "FFMA2" in line:
+            counts[fn] = counts.get(fn, 0) + 1
+        if fn and ("UTMALDG" in line or "UBLKCP" in line):
+            tma_ops[fn] = tma_ops.get(fn, 0) + 1
+    reinit_f32 = [f for f in counts if "k_reinit_tmaIf" in f]
+    advance_f32 = [f for f in counts if "k_advance_tmaIf" in f]
+    assert len(reinit_f32) == 5 and len(advance_f32) == 1, (reinit_f32, advance_f32)
+    for f in reinit_f32:
+        assert counts[f] == 18, (f, counts[f])
+    assert counts[advance_f32[0]] == 4, counts[advance_f32[0]]
+    # and the band kernels really are TMA kernels (cp.async.bulk.tensor -> UTMALDG, cp.async.bulk -> UBLKCP)
+    for f in reinit_f32 + advance_f32:
+        assert tma_ops.get(f, 0) >= 2, f

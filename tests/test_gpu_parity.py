@@ -344,3 +344,33 @@ def test_cfg5_reinit_tol():
         nxt, _ = orc.reinit_iter(g_conv, Nm, w.dtau, w.dx)
         inner = (Nm != 0) & (np.abs(g_conv) < w.gamma - 2 * w.dx)
         assert np.max(np.abs(nxt - g_conv)[inner]) < tol
+
+
+def test_selftest_packed_math_bit_identical():
+    """ls_selftest_math: the packed two-point fp32 arithmetic of the TMA band kernels equals the scalar
+    IEEE functions bit for bit on 3 x 2^24 random stencil pairs (band-like values, arbitrary bit
+    patterns, zeros, flat patches), with a dyadic and a non-dyadic dx."""
+    s = torch.cuda.current_stream().cuda_stream
+    for seed, dx in ((1, 1.0 / 1024), (2, 1.0 / 512), (3, 0.0137)):
+        bad = ls.ls_selftest_math(seed, 1 << 24, dx, 0.4 * dx, 3 * dx, 6 * dx, s)
+        assert bad == 0, f"{bad} of {4 << 24} packed results differ (seed {seed}, dx {dx})"
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("shape", [(20, 13, 40), (9, 24, 8), (33, 17, 64)])
+def test_tma_path_equals_oracle_exactly(shape, dtype):
+    """TMA-addressable ragged grids (nx*sizeof(T) % 16 == 0; partial bricks in y and z; band touching
+    the boundary): two free-running steps equal the oracle in every bit of every element (the contract
+    is 1e-5*dx / 1e-12*dx; the implementation follows O2-O7's operation order exactly, so == holds)."""
+    nz, ny, nx = shape
+    dx = 1.0 / 32
+    phi, F = _random_band_field(shape, dtype, 77, dx)
+    want, upd = orc.step(phi, F, dx, 0.4 * dx, 0.5 * dx, 3 * dx, 6 * dx, 5, 2)
+    for rebuild in (ls.LS_REBUILD_FULL, ls.LS_REBUILD_INCREMENTAL):
+        with Ctx(shape, dtype) as ctx:
+            d_phi, d_F = to_dev(phi), to_dev(F)
+            ls.ls_step(ctx, d_phi, d_F, ls.make_params(dx, 0.4 * dx, 0.5 * dx, 3 * dx, 6 * dx, 5, rebuild), 2)
+            got = d_phi.cpu().numpy()
+            updates, _, _ = ls.ls_stats(ctx)
+        assert updates == upd
+        assert np.array_equal(got, want.astype(dtype)), f"max err {max_err_dx(got, want, dx)} dx"
