@@ -270,10 +270,13 @@ k_reinit_tma(const __grid_constant__ CUtensorMap tm_src, T* __restrict__ dst, Ge
         // from the tile (iteration k), results go to the out brick (iteration k+1).
 #pragma unroll
         for (int r = 0; r < 2; ++r) {
-            const int e = 2 * (tid + r * kThreads);
+            // lane l of warp w takes list entries e and e + 32: each shared-memory load of a warp then covers
+            // 32 CONSECUTIVE points (4 brick rows), the least bank-conflicting set this tile pitch allows
+            const int e = r * 2 * kThreads + 64 * w + lane;
             if (e < total) {
-                uint2 ent = *reinterpret_cast<const uint2*>(list + e);
-                if (e + 1 >= total) ent.y = ent.x;   // odd tail: evaluate the last point twice
+                uint2 ent;
+                ent.x = list[e];
+                ent.y = e + 32 < total ? list[e + 32] : ent.x;   // tail: evaluate the point twice
                 const int o0 = (int)(ent.x & 0xffffu), o1 = (int)(ent.y & 0xffffu);
                 Two<T> u = reinit_pair<T>(tile, o0, o1, SY, SZ, p);
                 if (RESIDUAL) rmax = fmax(rmax, fmax(mag(u.x - tile[o0]), mag(u.y - tile[o1])));
@@ -339,7 +342,7 @@ k_advance_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant_
     extern __shared__ __align__(128) unsigned char smem[];
     uint32_t* list = reinterpret_cast<uint32_t*>(smem + kStages * S::BYTES);
     T* outb = reinterpret_cast<T*>(smem + kStages * S::BYTES + kListBytes);
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int count = *count_ptr;
     const int G = gridDim.x;
     const int mine = (int)blockIdx.x < count ? (count - (int)blockIdx.x + G - 1) / G : 0;
@@ -393,10 +396,11 @@ k_advance_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant_
         if (tid == 0 && p_left > 0) issue();
 #pragma unroll
         for (int r = 0; r < 2; ++r) {
-            const int e = 2 * (tid + r * kThreads);
+            const int e = r * 2 * kThreads + 64 * w + lane;   // entries e and e + 32, see k_reinit_tma
             if (e < total) {
-                uint2 ent = *reinterpret_cast<const uint2*>(list + e);
-                if (e + 1 >= total) ent.y = ent.x;
+                uint2 ent;
+                ent.x = list[e];
+                ent.y = e + 32 < total ? list[e + 32] : ent.x;
                 const Two<T> u = advance_pair<T>(tile, (int)(ent.x & 0xffffu), (int)(ent.y & 0xffffu), SY, SZ,
                                                  Fb[ent.x >> 16], Fb[ent.y >> 16], p);
                 outb[ent.x >> 16] = u.x;
