@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstddef>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <new>
@@ -541,17 +542,24 @@ ls_status ls_selftest_math(void* cuda_stream, uint64_t seed, int64_t n, double d
     if (!mismatches || n < 0 || bad_band_params(dx, beta, gamma) || std::isinf(gamma)) return LS_ERR_ARG;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     unsigned long long* d = nullptr;
-    LS_CK(cudaMalloc((void**)&d, 8));
-    cudaError_t e = cudaMemsetAsync(d, 0, 8, s);
-    unsigned long long h = 0;
+    LS_CK(cudaMalloc((void**)&d, 16 + 32 * sizeof(float)));
+    float* dbg = reinterpret_cast<float*>(d + 2);
+    cudaError_t e = cudaMemsetAsync(d, 0, 16 + 32 * sizeof(float), s);
+    struct { unsigned long long n[2]; float v[32]; } out;
+    std::memset(&out, 0, sizeof out);
     if (e == cudaSuccess) {
-        ls::launch_selftest_math(seed, n, make_params<float>(dx, dt, beta, gamma), d, s);
+        ls::launch_selftest_math(seed, n, make_params<float>(dx, dt, beta, gamma), d, dbg, s);
         e = cudaPeekAtLastError();
     }
-    if (e == cudaSuccess) e = cudaMemcpyAsync(&h, d, 8, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&out, d, sizeof out, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     cudaFree(d);
     if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(e, "ls_selftest_math"); }
+    const unsigned long long h = out.n[0];
+    if (h && getenv("LS_SELFTEST_VERBOSE")) {   // first differing sample: stencils (zm ym xm c xp yp zp) x2, F, scalar / packed results
+        std::fprintf(stderr, "ls_selftest_math: %llu results differ; first sample:\n", h);
+        for (int k = 0; k < 26; ++k) std::fprintf(stderr, "  [%2d] %.9g (0x%08x)\n", k, out.v[k], *reinterpret_cast<unsigned*>(&out.v[k]));
+    }
     *mismatches = (int64_t)h;
     return LS_OK;
 }

@@ -108,8 +108,9 @@ bool launch_advance_tma(const T* phi, const T* F, T* out, const Geom& g, const S
                         const BandBuffers& bb, bool use_T_list, cudaStream_t s, int64_t* launches);
 
 // Bit-for-bit check of the packed pair arithmetic against the scalar functions on n random stencil pairs.
+// mismatches: 2 counters (differing results; differing samples); dbg: 26 floats of the first differing sample or null.
 void launch_selftest_math(uint64_t seed, int64_t n, const StencilParams<float>& p, unsigned long long* mismatches,
-                          cudaStream_t s);
+                          float* dbg, cudaStream_t s);
 
 int sm_count();
 

@@ -251,7 +251,7 @@ __device__ __forceinline__ bool same_bits(float a, float b) {
     return __float_as_uint(a) == __float_as_uint(b) || (a != a && b != b);
 }
 __global__ void __launch_bounds__(256) k_selftest_math(uint64_t seed, int64_t n, StencilParams<float> p,
-                                                       unsigned long long* mismatches) {
+                                                       unsigned long long* mismatches, float* dbg) {
     unsigned long long bad = 0;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         // line[h][3 + d], d in {-3: zm, -2: ym, -1: xm, 0: c, 1: xp, 2: yp, 3: zp}: a "tile" with strides sy = 2, sz = 3
@@ -283,7 +283,13 @@ __global__ void __launch_bounds__(256) k_selftest_math(uint64_t seed, int64_t n,
         const float a1 = advance_value<float, false>(b[3], b[2], b[4], b[1], b[5], b[0], b[6], f[1], p);
         const Two<float> rp = reinit_pair<float>(line, 3, 11, 2, 3, p);
         const Two<float> ap = advance_pair<float>(line, 3, 11, 2, 3, f[0], f[1], p);
-        bad += !same_bits(rp.x, r0) + !same_bits(rp.y, r1) + !same_bits(ap.x, a0) + !same_bits(ap.y, a1);
+        const int br = !same_bits(rp.x, r0) + !same_bits(rp.y, r1), ba = !same_bits(ap.x, a0) + !same_bits(ap.y, a1);
+        bad += br + ba;
+        if (dbg && (br | ba) && atomicAdd(mismatches + 1, 1ull) == 0) {   // first failing sample, for debugging
+            for (int k = 0; k < 16; ++k) dbg[k] = line[k];
+            dbg[16] = f[0]; dbg[17] = f[1]; dbg[18] = r0; dbg[19] = r1; dbg[20] = rp.x; dbg[21] = rp.y;
+            dbg[22] = a0; dbg[23] = a1; dbg[24] = ap.x; dbg[25] = ap.y;
+        }
     }
     if (bad) atomicAdd(mismatches, bad);
 }
@@ -299,8 +305,8 @@ bool tma_disabled() {
 }  // namespace
 
 void launch_selftest_math(uint64_t seed, int64_t n, const StencilParams<float>& p, unsigned long long* mismatches,
-                          cudaStream_t s) {
-    k_selftest_math<<<sm_count() * 8, 256, 0, s>>>(seed, n, p, mismatches);
+                          float* dbg, cudaStream_t s) {
+    k_selftest_math<<<sm_count() * 8, 256, 0, s>>>(seed, n, p, mismatches, dbg);
 }
 
 int sm_count() {

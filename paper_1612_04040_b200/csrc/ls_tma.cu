@@ -416,12 +416,6 @@ k_advance_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant_
 }
 
 int tma_grid(int ctas_per_sm) { return sm_count() * ctas_per_sm; }
-// Resident CTAs per SM by shared memory: 227 KB usable, 1 KB reserved per CTA, ~3 KB static (list, barriers).
-int ctas_per_sm(size_t dyn_smem) {
-    const int n = (int)((227 * 1024) / (dyn_smem + 4 * 1024));
-    return n < 1 ? 1 : (n > 12 ? 12 : n);
-}
-
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -457,9 +451,16 @@ bool make_map(CUtensorMap* m, const void* field, const Geom& g, int bx, int by, 
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// Persistent grid of a band kernel: the largest shared-memory carve-out, then as many CTAs as fit on an SM.
 template <typename K>
-void prefer_smem(K kernel) {
+int persistent_grid(K kernel, size_t dyn_smem) {
     cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kThreads, dyn_smem) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError();
+        per_sm = 1;
+    }
+    return tma_grid(per_sm);
 }
 
 }  // namespace
@@ -479,12 +480,10 @@ bool launch_reinit_tma(const T* src, T* dst, const Geom& g, const StencilParams<
     CUtensorMap tm;
     if (!make_map<T>(&tm, src, g, S::PX, kPY, kPY)) return false;
     const size_t shm = (size_t)kStages * S::BYTES + kListBytes + 512 * sizeof(T) + kBarBytes;
-    const int grid = tma_grid(ctas_per_sm(shm));
     const int32_t* cnt = &bb.counts->nN;
 #define LS_LAUNCH(C, R, E)                                                                                       \
     do {                                                                                                         \
-        static bool once = (prefer_smem(k_reinit_tma<T, C, R, E>), true);                                        \
-        (void)once;                                                                                              \
+        static const int grid = persistent_grid(k_reinit_tma<T, C, R, E>, shm);                                  \
         k_reinit_tma<T, C, R, E><<<grid, kThreads, shm, s>>>(tm, dst, g, p, bb.N_ids, bb.N_pos, cnt, bb.N_masks,    \
                                                              residual, bb.tmask, bb.flagT);                      \
     } while (0)
@@ -504,10 +503,8 @@ bool launch_advance_tma(const T* phi, const T* F, T* out, const Geom& g, const S
     using S = Stage<T, true>;
     CUtensorMap tm_phi, tm_F;
     if (!make_map<T>(&tm_phi, phi, g, S::PX, kPY, kPY) || !make_map<T>(&tm_F, F, g, 8, 8, 8)) return false;
-    static bool once = (prefer_smem(k_advance_tma<T>), true);
-    (void)once;
     const size_t shm = (size_t)kStages * S::BYTES + kListBytes + 512 * sizeof(T) + kBarBytes;
-    const int grid = tma_grid(ctas_per_sm(shm));
+    static const int grid = persistent_grid(k_advance_tma<T>, shm);
     if (use_T_list)
         k_advance_tma<T><<<grid, kThreads, shm, s>>>(tm_phi, tm_F, out, g, p, bb.T_ids, bb.T_pos, &bb.counts->nT,
                                                      bb.T_masks, nullptr, nullptr);
