@@ -345,6 +345,10 @@ ls_status ls_band_export(ls_ctx* c, int32_t* T_ids, uint64_t* T_masks, int32_t* 
     ls_status st = ls_band_counts(c, nullptr, nullptr, &nT, &nN);
     if (st != LS_OK) return st;
     cudaStream_t s = c->stream;
+    if (N_masks) {   // list-ordered copy of the dense per-brick N masks
+        ls::launch_gather_masks(c->bb, s, &c->launches);
+        LS_CK_LAUNCH();
+    }
     if (T_ids && nT) LS_CK(cudaMemcpyAsync(T_ids, c->bb.T_ids, (size_t)nT * 4, cudaMemcpyDeviceToHost, s));
     if (T_masks && nT) LS_CK(cudaMemcpyAsync(T_masks, c->bb.T_masks, (size_t)nT * 64, cudaMemcpyDeviceToHost, s));
     if (N_ids && nN) LS_CK(cudaMemcpyAsync(N_ids, c->bb.N_ids, (size_t)nN * 4, cudaMemcpyDeviceToHost, s));
@@ -558,7 +562,11 @@ ls_status ls_selftest_math(void* cuda_stream, uint64_t seed, int64_t n, double d
     const unsigned long long h = out.n[0];
     if (h && getenv("LS_SELFTEST_VERBOSE")) {   // first differing sample: stencils (zm ym xm c xp yp zp) x2, F, scalar / packed results
         std::fprintf(stderr, "ls_selftest_math: %llu results differ; first sample:\n", h);
-        for (int k = 0; k < 26; ++k) std::fprintf(stderr, "  [%2d] %.9g (0x%08x)\n", k, out.v[k], *reinterpret_cast<unsigned*>(&out.v[k]));
+        for (int k = 0; k < 26; ++k) {
+            unsigned bits;
+            std::memcpy(&bits, &out.v[k], 4);
+            std::fprintf(stderr, "  [%2d] %.9g (0x%08x)\n", k, out.v[k], bits);
+        }
     }
     *mismatches = (int64_t)h;
     return LS_OK;

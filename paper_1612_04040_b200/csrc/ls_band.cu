@@ -100,43 +100,67 @@ __device__ __forceinline__ uint64_t domain_word(const Geom& g, int bx, int by, i
     return w;
 }
 
-// eq. 11 (R6): N = T or any in-domain face neighbour in T.  One thread per (brick, lz).
+// eq. 11 (R6): N = T or any in-domain face neighbour in T.  One thread per brick: 7 flag bytes decide
+// whether the brick can hold N points at all (3 % of the bricks of cfg 4 can); only those touch masks.
+// Also counts |T| and |N| into the accumulators of Counts (integer adds commute: order independent).
 __global__ void __launch_bounds__(256) k_dilate(Geom g, const uint64_t* __restrict__ tmask,
                                                 const uint8_t* __restrict__ flagT, uint64_t* __restrict__ nmask,
-                                                uint8_t* __restrict__ flagN) {
-    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const int b = (int)(t >> 3), lz = (int)(t & 7);
-    const bool valid = b < g.nbricks;
-    uint64_t n = 0;
-    if (valid) {
+                                                uint8_t* __restrict__ flagN, Counts* __restrict__ counts) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned ptsT = 0, ptsN = 0;
+    if (b < g.nbricks) {
         const int bx = b % g.NBx, by = (b / g.NBx) % g.NBy, bz = b / (g.NBx * g.NBy);
         const int sx = 1, sy = g.NBx, sz = g.NBx * g.NBy;
         const bool self = flagT[b] != 0;
         const bool xm = bx > 0 && flagT[b - sx], xp = bx < g.NBx - 1 && flagT[b + sx];
         const bool ym = by > 0 && flagT[b - sy], yp = by < g.NBy - 1 && flagT[b + sy];
         const bool zm = bz > 0 && flagT[b - sz], zp = bz < g.NBz - 1 && flagT[b + sz];
+        bool any = false;
         if (self | xm | xp | ym | yp | zm | zp) {
-            const uint64_t* own = tmask + (int64_t)b * 8;
-            if (self) {
-                const uint64_t w = own[lz];
-                n = w | ((w << 1) & ~COL0) | ((w >> 1) & ~COL7) | (w << 8) | (w >> 8);
-                if (lz > 0) n |= own[lz - 1];
-                if (lz < 7) n |= own[lz + 1];
+            uint64_t own[8];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                ulonglong2 v = make_ulonglong2(0ull, 0ull);
+                if (self) v = reinterpret_cast<const ulonglong2*>(tmask + (int64_t)b * 8)[i];
+                own[2 * i] = v.x;
+                own[2 * i + 1] = v.y;
             }
-            if (lz == 0 && zm) n |= tmask[(int64_t)(b - sz) * 8 + 7];
-            if (lz == 7 && zp) n |= tmask[(int64_t)(b + sz) * 8 + 0];
-            if (xm) n |= (tmask[(int64_t)(b - sx) * 8 + lz] >> 7) & COL0;   // their lx=7 -> our lx=0
-            if (xp) n |= (tmask[(int64_t)(b + sx) * 8 + lz] & COL0) << 7;   // their lx=0 -> our lx=7
-            if (ym) n |= tmask[(int64_t)(b - sy) * 8 + lz] >> 56;           // their ly=7 -> our ly=0
-            if (yp) n |= (tmask[(int64_t)(b + sy) * 8 + lz] & 0xffull) << 56;
-            n &= domain_word(g, bx, by, bz, lz);
+            const uint64_t below = zm ? tmask[(int64_t)(b - sz) * 8 + 7] : 0ull;
+            const uint64_t above = zp ? tmask[(int64_t)(b + sz) * 8 + 0] : 0ull;
+            const uint64_t* txm = tmask + (int64_t)(b - sx) * 8;
+            const uint64_t* txp = tmask + (int64_t)(b + sx) * 8;
+            const uint64_t* tym = tmask + (int64_t)(b - sy) * 8;
+            const uint64_t* typ = tmask + (int64_t)(b + sy) * 8;
+            uint64_t out[8];
+#pragma unroll
+            for (int lz = 0; lz < 8; ++lz) {
+                const uint64_t w = own[lz];
+                uint64_t n = w | ((w << 1) & ~COL0) | ((w >> 1) & ~COL7) | (w << 8) | (w >> 8);
+                n |= lz > 0 ? own[lz - 1] : below;
+                n |= lz < 7 ? own[lz + 1] : above;
+                if (xm) n |= (txm[lz] >> 7) & COL0;   // their lx=7 -> our lx=0
+                if (xp) n |= (txp[lz] & COL0) << 7;   // their lx=0 -> our lx=7
+                if (ym) n |= tym[lz] >> 56;           // their ly=7 -> our ly=0
+                if (yp) n |= (typ[lz] & 0xffull) << 56;
+                n &= domain_word(g, bx, by, bz, lz);
+                out[lz] = n;
+                any = any || n != 0;
+                ptsN += __popcll(n);
+                ptsT += __popcll(w);
+            }
+            if (any) {
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    reinterpret_cast<ulonglong2*>(nmask + (int64_t)b * 8)[i] = make_ulonglong2(out[2 * i], out[2 * i + 1]);
+            }
         }
+        flagN[b] = any ? 1 : 0;
     }
-    const unsigned nz_lanes = __ballot_sync(0xffffffffu, n != 0);
-    const bool brick_any = ((nz_lanes >> (threadIdx.x & 24)) & 0xffu) != 0;
-    if (valid) {
-        if (brick_any) nmask[(int64_t)b * 8 + lz] = n;
-        if (lz == 0) flagN[b] = brick_any ? 1 : 0;
+    ptsT = __reduce_add_sync(0xffffffffu, ptsT);
+    ptsN = __reduce_add_sync(0xffffffffu, ptsN);
+    if ((threadIdx.x & 31) == 0) {
+        if (ptsT) atomicAdd(&counts->acc_T, (unsigned long long)ptsT);
+        if (ptsN) atomicAdd(&counts->acc_N, (unsigned long long)ptsN);
     }
 }
 
@@ -226,26 +250,13 @@ __global__ void __launch_bounds__(1024) k_scan_partials(int32_t* __restrict__ pa
         }
         __syncthreads();
     }
-    if (threadIdx.x == 0) { counts->nT_pts = 0; counts->nN_pts = 0; }
 }
 
-__device__ __forceinline__ int copy_mask(const uint64_t* __restrict__ src, uint64_t* __restrict__ dst) {
-    int pts = 0;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const ulonglong2 v = reinterpret_cast<const ulonglong2*>(src)[i];
-        reinterpret_cast<ulonglong2*>(dst)[i] = v;
-        pts += __popcll(v.x) + __popcll(v.y);
-    }
-    return pts;
-}
-
+// Ordered scatter of the brick ids (and packed positions) of the three lists.
 __global__ void __launch_bounds__(kScanThreads) k_scatter(const uint8_t* __restrict__ fT, const uint8_t* __restrict__ fN,
                                                           const uint8_t* __restrict__ fP,
                                                           const int32_t* __restrict__ partials, int npartials,
-                                                          const uint64_t* __restrict__ tmask,
-                                                          const uint64_t* __restrict__ nmask, BandBuffers bb,
-                                                          Geom g) {
+                                                          BandBuffers bb, Geom g) {
     __shared__ int wtot[3][kScanThreads / 32];
     const int base = blockIdx.x * kScanTile + threadIdx.x * kItemsPerThread;
     uint32_t m[3];
@@ -265,41 +276,37 @@ __global__ void __launch_bounds__(kScanThreads) k_scatter(const uint8_t* __restr
         excl[l] = incl - c;
     }
     __syncthreads();
+    if ((m[0] | m[1] | m[2]) == 0) return;   // no barrier or warp collective below
 #pragma unroll
     for (int l = 0; l < 3; ++l) {
         int off = partials[l * npartials + blockIdx.x];
         for (int i = 0; i < w; ++i) off += wtot[l][i];
         excl[l] += off;
     }
-    int ptsT = 0, ptsN = 0;
     int bx = base % g.NBx, by = (base / g.NBx) % g.NBy, bz = base / (g.NBx * g.NBy);
     for (int i = 0; i < kItemsPerThread; ++i) {
         const int b = base + i;
         const int pos = bx | (by << g.pos_sy) | (bz << g.pos_sz);
         if (++bx == g.NBx) { bx = 0; if (++by == g.NBy) { by = 0; ++bz; } }
-        if ((m[0] >> i) & 1u) {
-            bb.T_ids[excl[0]] = b;
-            bb.T_pos[excl[0]] = pos;
-            ptsT += copy_mask(tmask + (int64_t)b * 8, bb.T_masks + (int64_t)excl[0] * 8);
-            ++excl[0];
-        }
-        if ((m[1] >> i) & 1u) {
-            bb.N_ids[excl[1]] = b;
-            bb.N_pos[excl[1]] = pos;
-            ptsN += copy_mask(nmask + (int64_t)b * 8, bb.N_masks + (int64_t)excl[1] * 8);
-            ++excl[1];
-        }
+        if ((m[0] >> i) & 1u) { bb.T_ids[excl[0]] = b; bb.T_pos[excl[0]++] = pos; }
+        if ((m[1] >> i) & 1u) { bb.N_ids[excl[1]] = b; bb.N_pos[excl[1]++] = pos; }
         if ((m[2] >> i) & 1u) { bb.U_ids[excl[2]] = b; bb.U_pos[excl[2]++] = pos; }
-    }
-    ptsT = warp_sum(ptsT);
-    ptsN = warp_sum(ptsN);
-    if (lane == 0) {  // integer adds commute: the totals do not depend on arrival order
-        if (ptsT) atomicAdd(&bb.counts->nT_pts, (unsigned long long)ptsT);
-        if (ptsN) atomicAdd(&bb.counts->nN_pts, (unsigned long long)ptsN);
     }
 }
 
+// List-ordered copies of the dense masks (ls_band_export only): one thread per (list entry, word).
+__global__ void __launch_bounds__(256) k_gather_masks(const int32_t* __restrict__ ids, const int32_t* __restrict__ count_ptr,
+                                                      const uint64_t* __restrict__ dense, uint64_t* __restrict__ out) {
+    const int64_t n = (int64_t)*count_ptr * 8;
+    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (int64_t)gridDim.x * blockDim.x)
+        out[t] = dense[(int64_t)ids[t >> 3] * 8 + (t & 7)];
+}
+
 __global__ void k_finalize(Counts* counts, int iters, int count_step) {
+    counts->nT_pts = counts->acc_T;
+    counts->nN_pts = counts->acc_N;
+    counts->acc_T = 0;
+    counts->acc_N = 0;
     if (count_step) {
         counts->updates += counts->nT_pts + (unsigned long long)iters * counts->nN_pts;
         counts->steps += 1;
@@ -322,14 +329,20 @@ void launch_classify(const T* phi, const Geom& g, T gamma, const BandBuffers& bb
 
 void launch_dilate_compact(const Geom& g, const BandBuffers& bb, int iters, bool count_step, cudaStream_t s,
                            int64_t* launches) {
-    const int64_t nthreads = (int64_t)g.nbricks * 8;
-    k_dilate<<<(unsigned)((nthreads + 255) / 256), 256, 0, s>>>(g, bb.tmask, bb.flagT, bb.nmask, bb.flagN);
+    k_dilate<<<(unsigned)((g.nbricks + 255) / 256), 256, 0, s>>>(g, bb.tmask, bb.flagT, bb.nmask, bb.flagN, bb.counts);
     k_count<<<bb.npartials, kScanThreads, 0, s>>>(bb.flagT, bb.flagN, bb.flagNprev, bb.partials, bb.npartials);
     k_scan_partials<<<1, 1024, 0, s>>>(bb.partials, bb.npartials, bb.counts);
-    k_scatter<<<bb.npartials, kScanThreads, 0, s>>>(bb.flagT, bb.flagN, bb.flagNprev, bb.partials, bb.npartials,
-                                                    bb.tmask, bb.nmask, bb, g);
+    k_scatter<<<bb.npartials, kScanThreads, 0, s>>>(bb.flagT, bb.flagN, bb.flagNprev, bb.partials, bb.npartials, bb, g);
     k_finalize<<<1, 1, 0, s>>>(bb.counts, iters, count_step ? 1 : 0);
-    if (launches) *launches += 5;
+    // Snapshot of the T masks in list order: the last reinit sweep of an incremental step overwrites the
+    // dense T masks with those of phi^{n+1}, while ls_band_export reports the band of phi^n.
+    k_gather_masks<<<sm_count() * 2, 256, 0, s>>>(bb.T_ids, &bb.counts->nT, bb.tmask, bb.T_masks);
+    if (launches) *launches += 6;
+}
+
+void launch_gather_masks(const BandBuffers& bb, cudaStream_t s, int64_t* launches) {
+    k_gather_masks<<<sm_count() * 4, 256, 0, s>>>(bb.N_ids, &bb.counts->nN, bb.nmask, bb.N_masks);
+    if (launches) *launches += 1;
 }
 
 int scan_tile() { return kScanTile; }

@@ -26,6 +26,7 @@ struct Counts {
     int32_t nU;            // bricks in the U list (N of this step  ∪  N of the previous step)
     int32_t pad;
     unsigned long long nT_pts, nN_pts;  // |T|, |N|
+    unsigned long long acc_T, acc_N;    // accumulators of the build in flight (k_dilate), folded by k_finalize
     unsigned long long updates;         // sum over steps of |T| + iters*|N|
     unsigned long long steps;
 };
@@ -38,7 +39,7 @@ struct BandBuffers {
     uint8_t* flagN;    // [nbricks] N flags of the band being built
     uint8_t* flagNprev;// [nbricks] N flags of the previous step's band (all 0 at the start of a call)
     int32_t* T_ids;    // [nbricks]
-    uint64_t* T_masks; // [nbricks*8]
+    uint64_t* T_masks; // [nbricks*8] list-ordered snapshot of the T masks (export); N_masks: filled at export
     int32_t* N_ids;
     uint64_t* N_masks;
     int32_t* U_ids;
@@ -58,6 +59,10 @@ void launch_classify(const T* phi, const Geom& g, T gamma, const BandBuffers& bb
 // `iters` only feeds the update counter (|T| + iters*|N|).
 void launch_dilate_compact(const Geom& g, const BandBuffers& bb, int iters, bool count_step, cudaStream_t s,
                            int64_t* launches);
+
+// List-ordered copy N_masks of the dense N masks of the band last built (for ls_band_export; T_masks is
+// snapshotted by launch_dilate_compact).
+void launch_gather_masks(const BandBuffers& bb, cudaStream_t s, int64_t* launches);
 
 // ---- stencil kernels (ls_stencil.cu) --------------------------------------------------------
 template <typename T>

@@ -64,7 +64,7 @@ __global__ void __launch_bounds__(kBandThreads) k_advance_band(const T* __restri
             const int i = x0 + lx, j = y0 + ly, k = z0 + lz;
             if (i < g.nx && j < g.ny && k < g.nz) {
                 uint64_t w = 0;
-                if (has_T) w = list_masks ? list_masks[(int64_t)li * 8 + lz] : tmask[(int64_t)b * 8 + lz];
+                if (has_T) w = (list_masks ? list_masks : tmask)[(int64_t)b * 8 + lz];   // both dense per brick
                 const T c = LS_TILE(s, lx, ly, lz);
                 T v = c;
                 const int64_t at = g.idx(i, j, k);
@@ -103,7 +103,7 @@ __global__ void __launch_bounds__(kBandThreads) k_reinit_band(const T* __restric
         for (int h = 0; h < 2; ++h) {
             const int lz = lz0 + 4 * h;
             const int i = x0 + lx, j = y0 + ly, k = z0 + lz;
-            const uint64_t w = masks[(int64_t)li * 8 + lz];
+            const uint64_t w = masks[(int64_t)b * 8 + lz];   // dense per-brick N masks
             const unsigned rowbits = (unsigned)(w >> (ly * 8)) & 0xffu;
             const bool active = (rowbits >> lx) & 1u;
             bool tbit = false;
@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(kBandThreads) k_copy_clamp_band(const T* __res
         for (int h = 0; h < 2; ++h) {
             const int lz = lz0 + 4 * h;
             const int i = bx * 8 + lx, j = by * 8 + ly, k = bz * 8 + lz;
-            const uint64_t w = masks[(int64_t)li * 8 + lz];
+            const uint64_t w = masks[(int64_t)b * 8 + lz];   // dense per-brick N masks
             if (((w >> (ly * 8)) & 0xffull) != 0 && i < g.nx && j < g.ny && k < g.nz) {
                 const int64_t at = g.idx(i, j, k);
                 dst[at] = clamp_val(src[at], gamma);
@@ -327,7 +327,7 @@ void launch_advance_band(const T* phi, const T* F, T* out, const Geom& g, const 
         launch_advance_tma<T>(phi, F, out, g, p, bb, use_T_list, s, launches))
         return;
     if (use_T_list)
-        k_advance_band<T><<<band_grid(), kBandThreads, 0, s>>>(phi, F, out, g, p, bb.T_ids, &bb.counts->nT, bb.T_masks,
+        k_advance_band<T><<<band_grid(), kBandThreads, 0, s>>>(phi, F, out, g, p, bb.T_ids, &bb.counts->nT, bb.tmask,
                                                                nullptr, nullptr);
     else
         k_advance_band<T><<<band_grid(), kBandThreads, 0, s>>>(phi, F, out, g, p, bb.U_ids, &bb.counts->nU, nullptr,
@@ -353,7 +353,7 @@ void launch_reinit_band(const T* src, T* dst, const Geom& g, const StencilParams
     const int grid = band_grid();
     const int32_t* cnt = &bb.counts->nN;
 #define LS_LAUNCH(C, R, E)                                                                                        \
-    k_reinit_band<T, C, R, E><<<grid, kBandThreads, 0, s>>>(src, dst, g, p, bb.N_ids, cnt, bb.N_masks, residual, \
+    k_reinit_band<T, C, R, E><<<grid, kBandThreads, 0, s>>>(src, dst, g, p, bb.N_ids, cnt, bb.nmask, residual,   \
                                                             bb.tmask, bb.flagT)
     if (emit_T) LS_LAUNCH(true, false, true);
     else if (residual && clamp) LS_LAUNCH(true, true, false);
@@ -367,7 +367,7 @@ void launch_reinit_band(const T* src, T* dst, const Geom& g, const StencilParams
 template <typename T>
 void launch_copy_clamp_band(const T* src, T* dst, const Geom& g, T gamma, const BandBuffers& bb, cudaStream_t s,
                             int64_t* launches) {
-    k_copy_clamp_band<T><<<band_grid(), kBandThreads, 0, s>>>(src, dst, g, gamma, bb.N_ids, &bb.counts->nN, bb.N_masks);
+    k_copy_clamp_band<T><<<band_grid(), kBandThreads, 0, s>>>(src, dst, g, gamma, bb.N_ids, &bb.counts->nN, bb.nmask);
     if (launches) *launches += 1;
 }
 

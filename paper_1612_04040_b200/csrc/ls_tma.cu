@@ -243,7 +243,7 @@ k_reinit_tma(const __grid_constant__ CUtensorMap tm_src, T* __restrict__ dst, Ge
         const uint32_t st = smem_base + p_slot * S::BYTES, bar = bar_base + 8 * p_slot;
         mbar_expect_tx(bar, S::TILE_BYTES + 64);
         tma_load_3d(st, &tm_src, bar, h->x0 - XOFF, h->y0 - 1, h->z0 - 1);
-        bulk_load(st + S::OFF_MASK, masks + (int64_t)p_li * 8, 64, bar);
+        bulk_load(st + S::OFF_MASK, masks + (int64_t)b * 8, 64, bar);   // dense per-brick N masks
         p_li += G;
         p_slot = p_slot == kStages - 1 ? 0 : p_slot + 1;
         --p_left;
@@ -369,7 +369,7 @@ k_advance_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant_
         tma_load_3d(st, &tm_phi, bar, h->x0 - XOFF, h->y0 - 1, h->z0 - 1);
         if (has_T) {
             tma_load_3d(st + S::OFF_F, &tm_F, bar, h->x0, h->y0, h->z0);
-            const uint64_t* m = dense_tmask ? dense_tmask + (int64_t)b * 8 : list_masks + (int64_t)p_li * 8;
+            const uint64_t* m = (dense_tmask ? dense_tmask : list_masks) + (int64_t)b * 8;   // both dense per brick
             bulk_load(st + S::OFF_MASK, m, 64, bar);
         }
         p_li += G;
@@ -484,7 +484,7 @@ bool launch_reinit_tma(const T* src, T* dst, const Geom& g, const StencilParams<
 #define LS_LAUNCH(C, R, E)                                                                                       \
     do {                                                                                                         \
         static const int grid = persistent_grid(k_reinit_tma<T, C, R, E>, shm);                                  \
-        k_reinit_tma<T, C, R, E><<<grid, kThreads, shm, s>>>(tm, dst, g, p, bb.N_ids, bb.N_pos, cnt, bb.N_masks,    \
+        k_reinit_tma<T, C, R, E><<<grid, kThreads, shm, s>>>(tm, dst, g, p, bb.N_ids, bb.N_pos, cnt, bb.nmask,      \
                                                              residual, bb.tmask, bb.flagT);                      \
     } while (0)
     if (emit_T) LS_LAUNCH(true, false, true);
@@ -507,7 +507,7 @@ bool launch_advance_tma(const T* phi, const T* F, T* out, const Geom& g, const S
     static const int grid = persistent_grid(k_advance_tma<T>, shm);
     if (use_T_list)
         k_advance_tma<T><<<grid, kThreads, shm, s>>>(tm_phi, tm_F, out, g, p, bb.T_ids, bb.T_pos, &bb.counts->nT,
-                                                     bb.T_masks, nullptr, nullptr);
+                                                     bb.tmask, nullptr, nullptr);
     else
         k_advance_tma<T><<<grid, kThreads, shm, s>>>(tm_phi, tm_F, out, g, p, bb.U_ids, bb.U_pos, &bb.counts->nU,
                                                      nullptr, bb.tmask, bb.flagT);
