@@ -39,10 +39,13 @@ if str(ROOT) not in sys.path:
 
 METRIC = "narrow-band grid-point updates/sec (GLUPS)"
 UNIT = "GLUPS"
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
-NCU_TRAFFIC_BYTES = {"reinit": None}
-NCU_TRAFFIC_SOURCE = None
+# Per launch of the dominant kernel (k_reinit_tma<float,0,0,0>, cfg 4), from the committed `ncu --set full`
+# capture: dram__bytes_read.sum + dram__bytes_write.sum, and smsp__inst_executed.sum (warp instructions).
+NCU_TRAFFIC_BYTES = {"reinit": 213.6e6 + 69.8e6}
+NCU_WARP_INSTRUCTIONS = {"reinit": 70.23e6}
+NCU_TRAFFIC_SOURCE = "profiles/r1b_ncu_full_summary.txt (cfg 4, one capture; not re-measured per run)"
+# issue-slot peak: 148 SMs x 4 schedulers x 1 warp instruction / clock x SM clock
+ISSUE_SLOTS_PER_CLOCK = 148 * 4
 
 
 def parse_args():
@@ -289,9 +292,19 @@ def run_ours(args):
     nN_pts = out["prof_band"][1]   # |N| of the region's last step (the band moves < 1 cell per step)
     alg_bytes = 2 * esz * nN_pts + 68 * out["prof_band"][3]
     ach = alg_bytes / (r_ms / max(r_n, 1) * 1e-3) * 1e-9 if r_n else None
-    roofline = {"bound": "hbm", "kernel": "k_reinit_band (one Step 3 sweep)", "achieved": ach, "peak": peak,
+    is_cfg4 = w.name.startswith("cfg4") and w.nx == 1024
+    traffic = NCU_TRAFFIC_BYTES["reinit"] if is_cfg4 else None
+    sm_mhz = (out["clocks"] or {}).get("sm_mhz") or 1965.0
+    us = r_ms / max(r_n, 1) * 1e3
+    alu_peak = ISSUE_SLOTS_PER_CLOCK * sm_mhz * 1e6 * 1e-12          # T warp-instructions / s
+    alu_ach = (NCU_WARP_INSTRUCTIONS["reinit"] / (us * 1e-6) * 1e-12) if (is_cfg4 and r_n) else None
+    roofline_alu = {"bound": "alu", "kernel": "k_reinit_tma (one Step 3 sweep)", "achieved": alu_ach, "peak": alu_peak,
+                    "unit": "T warp-instructions/s", "frac": (alu_ach / alu_peak) if alu_ach else None,
+                    "note": "issue slots: executed warp instructions per launch (ncu capture) / live launch duration; "
+                            "peak = 148 SMs x 4 schedulers x SM clock sampled during the run (DESIGN.md section 6)"}
+    roofline = {"bound": "hbm", "kernel": "k_reinit_tma (one Step 3 sweep)", "achieved": ach, "peak": peak,
                 "peak_source": peak_src, "unit": "GB/s", "frac": (ach / peak) if ach else None,
-                "traffic": NCU_TRAFFIC_BYTES["reinit"], "traffic_source": NCU_TRAFFIC_SOURCE,
+                "traffic": traffic, "traffic_source": NCU_TRAFFIC_SOURCE if traffic else None,
                 "algorithmic_bytes_per_launch": alg_bytes, "us_per_launch": r_ms / max(r_n, 1) * 1e3,
                 "frac_of_8TBps_nominal": (ach / 8000.0) if ach else None}
     cpu = None
@@ -310,7 +323,7 @@ def run_ours(args):
                    "l2": "inputs larger than L2 (fields 4 GiB each; one band sweep touches ~0.3 GB > 126 MB L2)"
                    if w.n_points * esz > 512e6 else "working set fits L2 (small config): not a bandwidth number"},
         "clocks": out["clocks"], "e2e": out.get("e2e"), "gpu_launches": out["launches"],
-        "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu,
+        "roofline": roofline, "roofline_alu": roofline_alu, "kernels": kernels, "cpu_baseline": cpu,
     }
     print(json.dumps(line), flush=True)
     if world > 1:
