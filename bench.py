@@ -118,6 +118,17 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def aggregate_over_ranks(ms: float, updates: int, world: int, device: str = "cuda"):
+    """N > 1 is replicas only: -> (max-over-ranks milliseconds, whole-job updates).
+    The only collective of the bench: one MAX all-reduce of the timing (every rank does `updates`)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item()), world * updates
+
+
 def make_workload(args):
     from paper_1612_04040_b200 import inputs
     w = inputs.config(args.config, n=args.n)
@@ -237,11 +248,8 @@ def run_ours(args):
         updates, steps_done, launches = ls.ls_stats(ctx)
         assert steps_done == K
         nT, nN, bT, bN = ls.ls_band_counts(ctx)   # band of the last step
-        tmax = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        ms_max = float(tmax.item())
-        out.update(ms=ms_max, updates=updates, launches=launches, band=(nT, nN, bT, bN), clocks=clocks)
+        ms_max, job_updates = aggregate_over_ranks(ms, updates, world)
+        out.update(ms=ms_max, updates=updates, job_updates=job_updates, launches=launches, band=(nT, nN, bT, bN), clocks=clocks)
 
         # ---- same K-step region again with per-kernel event brackets (roofline / breakdown) ----
         if rank == 0:
@@ -279,7 +287,7 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
-    value = world * out["updates"] / (out["ms"] * 1e-3) * 1e-9
+    value = out["job_updates"] / (out["ms"] * 1e-3) * 1e-9
     peak, peak_src = peaks()
     prof = out["prof"]
     total_prof_ms = sum(ms for ms, _ in prof.values()) or 1.0
