@@ -272,7 +272,8 @@ k_reinit_tma(const __grid_constant__ CUtensorMap tm_src, T* __restrict__ dst, Ge
         for (int r = 0; r < 2; ++r) {
             // lane l of warp w takes list entries e and e + 32: each shared-memory load of a warp then covers
             // 32 CONSECUTIVE points (4 brick rows), the least bank-conflicting set this tile pitch allows
-            const int e = r * 2 * kThreads + 64 * w + lane;
+            // round 1 deals its (usually few) entries to warp 3 first: warp 0 also runs the producer
+            const int e = r * 2 * kThreads + 64 * (r ? kThreads / 32 - 1 - w : w) + lane;
             if (e < total) {
                 uint2 ent;
                 ent.x = list[e];
@@ -396,7 +397,7 @@ k_advance_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant_
         if (tid == 0 && p_left > 0) issue();
 #pragma unroll
         for (int r = 0; r < 2; ++r) {
-            const int e = r * 2 * kThreads + 64 * w + lane;   // entries e and e + 32, see k_reinit_tma
+            const int e = r * 2 * kThreads + 64 * (r ? kThreads / 32 - 1 - w : w) + lane;   // see k_reinit_tma
             if (e < total) {
                 uint2 ent;
                 ent.x = list[e];
