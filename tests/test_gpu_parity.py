@@ -374,3 +374,120 @@ def test_tma_path_equals_oracle_exactly(shape, dtype):
             updates, _, _ = ls.ls_stats(ctx)
         assert updates == upd
         assert np.array_equal(got, want.astype(dtype)), f"max err {max_err_dx(got, want, dx)} dx"
+
+
+# ---------------------------------------------------------------------------------------------
+# Full BASELINE.json sizes, in the launch configuration bench.py times (one unchained step, then
+# chained incremental steps).  The oracle cannot sweep 1024^3 in seconds, so it recomputes CROPS:
+# a step reads at most 1 (Advance) + 5 (sweeps) + 2 (tube N around T) = 8 cells around a point, so
+# after s steps a crop with a margin of 8 s cells reproduces the full-grid values in its interior
+# exactly (where a crop face coincides with the domain boundary, edge replicate is the true rule and no
+# margin is needed).  Interiors are brick aligned so band masks can be compared bit for bit too.
+# ---------------------------------------------------------------------------------------------
+def _crop_boxes(n, centres, size, margin):
+    """-> list of (origin, interior lo, interior hi) per axis-tuple; origins multiples of 8, inside the grid."""
+    boxes = []
+    for c in centres:
+        org = [int(np.clip((int(ci) - size // 2) // 8 * 8, 0, n - size)) for ci in c]   # (z, y, x)
+        lo = [0 if o == 0 else margin for o in org]
+        hi = [size if o + size == n else size - margin for o in org]
+        boxes.append((org, lo, hi))
+    return boxes
+
+
+def _masks_from_export(ids, words, NB, org, lo, hi):
+    """Point mask (bool) of the crop interior from a brick list export (ids ascending, words [n, 8])."""
+    out = {}
+    for b, w in zip(ids.tolist(), words):
+        out[b] = w
+    shape = tuple(h - l for l, h in zip(lo, hi))
+    m = np.zeros(shape, bool)
+    for bz in range((org[0] + lo[0]) // 8, (org[0] + hi[0]) // 8):
+        for by in range((org[1] + lo[1]) // 8, (org[1] + hi[1]) // 8):
+            for bx in range((org[2] + lo[2]) // 8, (org[2] + hi[2]) // 8):
+                w = out.get((bz * NB + by) * NB + bx)
+                if w is None:
+                    continue
+                bits = np.unpackbits(w.view(np.uint8), bitorder="little").reshape(8, 8, 8).astype(bool)
+                z0, y0, x0 = bz * 8 - org[0] - lo[0], by * 8 - org[1] - lo[1], bx * 8 - org[2] - lo[2]
+                m[z0:z0 + 8, y0:y0 + 8, x0:x0 + 8] = bits
+    return m
+
+
+@pytest.mark.parametrize("cfg", [4, 3])
+def test_full_size_band_steps_sampled(cfg):
+    w = inputs.config(cfg)
+    n, steps, size = w.nx, 3, 112
+    margin = 8 * steps
+    if cfg == 4:   # torus R = 0.3, r = 0.1: outer / inner equator, top, and a diagonal point of the tube
+        pts = [(0.5, 0.5, 0.9), (0.5, 0.7, 0.5), (0.6, 0.5, 0.8), (0.5 + 0.1 * 0.6, 0.5 + 0.38 * 0.6, 0.5 + 0.38 * 0.8)]
+    else:          # cfg 3: +x pole of the first three seeded spheres, and the grid corner
+        u = inputs.uniform01(3001, 0, 4 * 32).reshape(32, 4)
+        pts = [(0.1 + 0.8 * u[s, 2], 0.1 + 0.8 * u[s, 1], 0.1 + 0.8 * u[s, 0] + 0.03 + 0.09 * u[s, 3]) for s in range(3)]
+        pts.append((0.0, 0.0, 0.0))
+    boxes = _crop_boxes(n, [[p * n for p in pt] for pt in pts], size, margin)
+    p0 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, ls.LS_REBUILD_INCREMENTAL, 0)
+    p1 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, ls.LS_REBUILD_INCREMENTAL, 1)
+    with Ctx(w.shape, w.dtype) as ctx:
+        d_phi, d_F = to_dev(w.phi), to_dev(w.F)
+        # band of phi^0 at full size: |T| against torch's own count and (cfg 4) the closed form of I12
+        ls.ls_build_band(ctx, d_phi, w.dx, w.gamma)
+        nT0 = ls.ls_band_counts(ctx)[0]
+        assert nT0 == int((d_phi.abs() < np.float32(w.gamma)).sum().item())
+        if cfg == 4:
+            assert abs(nT0 / n ** 3 - 4 * np.pi ** 2 * 0.3 * 0.1 * 12 * w.dx) < 0.01 * 0.0139
+        ls.ls_step(ctx, d_phi, d_F, p0, 1)
+        ls.ls_step(ctx, d_phi, d_F, p1, steps - 1)
+        nT, nN, bT, bN = ls.ls_band_counts(ctx)      # band of the last step (built from phi^{steps-1})
+        T_ids, T_w, N_ids, N_w = ls.ls_band_export(ctx)
+        gamma32 = np.float32(w.gamma)
+        assert float(d_phi.abs().max().item()) <= gamma32                       # eq. 10 everywhere (I4)
+        got = d_phi.cpu().numpy()
+    assert len(T_ids) == bT and len(N_ids) == bN and np.all(np.diff(N_ids) > 0) and np.all(np.diff(T_ids) > 0)
+    assert int(np.unpackbits(T_w.view(np.uint8)).sum()) == nT and int(np.unpackbits(N_w.view(np.uint8)).sum()) == nN
+    checked = 0
+    for org, lo, hi in boxes:
+        sl = tuple(slice(o, o + size) for o in org)
+        inner = tuple(slice(l, h) for l, h in zip(lo, hi))
+        phi_c, F_c = np.ascontiguousarray(w.phi[sl]), np.ascontiguousarray(w.F[sl])
+        prev, _ = orc.step(phi_c, F_c, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, steps - 1)
+        want, _ = orc.step(prev, F_c, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, 1)
+        g = got[sl][inner]
+        assert np.array_equal(g, want[inner]), f"crop at {org}: max err {max_err_dx(g, want[inner], w.dx)} dx"
+        Tm, Nm = orc.band_masks(prev, w.gamma)       # the band the last step used
+        assert np.array_equal(_masks_from_export(T_ids, T_w, n // 8, org, lo, hi), Tm[inner] != 0)
+        assert np.array_equal(_masks_from_export(N_ids, N_w, n // 8, org, lo, hi), Nm[inner] != 0)
+        checked += int((Nm[inner] != 0).sum())
+        # points off N hold exactly +-gamma after a step (I4)
+        off = (Nm[inner] == 0)
+        assert np.all(np.abs(g[off]) == gamma32)
+    assert checked > 50000   # the crops really sit on the band
+
+
+def test_full_size_cfg5_reinit_sampled():
+    """cfg 5 at 512^3 fp64: 40 sweeps of ls_reinit on the band of phi^0, crops recomputed by the oracle
+    (margin 40 + 2 cells), bit for bit; and the residual rule of ls_reinit_tol at full size."""
+    w = inputs.config(5)
+    n, iters, size = w.nx, 40, 128
+    margin = 48
+    pts = [(0.5, 0.25, 1 / 3), (0.5, 0.75, 2 / 3), (0.5, 0.0, 0.0)]   # nodes of the wave (z = 0.5); one at the domain edge
+    boxes = _crop_boxes(n, [[p * n for p in pt] for pt in pts], size, margin)
+    with Ctx(w.shape, w.dtype) as ctx:
+        d_phi = to_dev(w.phi)
+        d = torch.empty_like(d_phi)
+        ls.ls_build_band(ctx, d_phi, w.dx, w.gamma)
+        nT = ls.ls_band_counts(ctx)[0]
+        assert nT == int((d_phi.abs() < w.gamma).sum().item())
+        assert abs(nT / (16 * n * n) - 1.0) < 0.08          # 16 n^2 without the noise factor (I12), ~ +3 % with it
+        ls.ls_reinit(ctx, d, d_phi, w.dtau, w.dx, w.gamma, iters)
+        got = d.cpu().numpy()
+        k, r, conv = ls.ls_reinit_tol(ctx, d, d_phi, w.dtau, w.dx, w.gamma, w.tol, 60, 20)
+        assert (k, conv) == (60, False) and r > 100 * w.tol   # far from the 1e-10 steady state after 60 sweeps (R13)
+    for org, lo, hi in boxes:
+        sl = tuple(slice(o, o + size) for o in org)
+        inner = tuple(slice(l, h) for l, h in zip(lo, hi))
+        phi_c = np.ascontiguousarray(w.phi[sl])
+        _, Nm = orc.band_masks(phi_c, w.gamma)
+        want = orc.reinit(phi_c, Nm, w.dtau, w.dx, w.gamma, iters)
+        assert np.array_equal(got[sl][inner], want[inner]), f"crop at {org}"
+        assert (Nm[inner] != 0).sum() > 10000
