@@ -172,7 +172,7 @@ ls_status ls_profile_reset(ls_ctx* ctx);
  * FADD2 / FMUL2 / FFMA2 instructions and hand-sequenced correctly rounded sqrt / divide; this runs both
  * that path and the plain scalar IEEE path (eq. 3-8 and eq. 12-13) on `n` pairs of seeded random 7-point
  * stencils (band-like values, arbitrary bit patterns, zeros, flat patches) on the current device and
- * returns how many of the 4n results differ in any bit (NaN == NaN).  Must be 0.  Runs on `cuda_stream`
+ * returns how many of the 6n results (reinit, band Advance, dense Advance) differ in any bit (NaN == NaN).  Must be 0.  Runs on `cuda_stream`
  * and synchronises it.  HOST out-pointer. */
 ls_status ls_selftest_math(void* cuda_stream, uint64_t seed, int64_t n, double dx, double dt, double beta,
                            double gamma, int64_t* mismatches);

@@ -102,7 +102,7 @@ def test_advance_band_parity(shape, dtype):
 
 
 @pytest.mark.parametrize("dtype", [np.float32, np.float64])
-@pytest.mark.parametrize("shape", [(9, 13, 20), (32, 32, 32), (40, 24, 72)])
+@pytest.mark.parametrize("shape", [(9, 13, 20), (32, 32, 32), (40, 24, 72), (5, 6, 7), (3, 9, 130)])
 def test_advance_dense_parity(shape, dtype):
     dx = 1.0 / 32
     phi, F = _random_band_field(shape, dtype, 31, dx)
@@ -353,7 +353,7 @@ def test_selftest_packed_math_bit_identical():
     s = torch.cuda.current_stream().cuda_stream
     for seed, dx in ((1, 1.0 / 1024), (2, 1.0 / 512), (3, 0.0137)):
         bad = ls.ls_selftest_math(seed, 1 << 24, dx, 0.4 * dx, 3 * dx, 6 * dx, s)
-        assert bad == 0, f"{bad} of {4 << 24} packed results differ (seed {seed}, dx {dx})"
+        assert bad == 0, f"{bad} of {6 << 24} packed results differ (seed {seed}, dx {dx})"
 
 
 @pytest.mark.parametrize("dtype", [np.float32, np.float64])
