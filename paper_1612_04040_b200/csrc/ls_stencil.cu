@@ -214,20 +214,32 @@ __global__ void __launch_bounds__(256) k_advance_dense2(const float* __restrict_
     const int jm = max(jc - 1, 0), jp = min(jc + 1, g.ny - 1);
     const int il = max(ic - 1, 0), ir = min(ic + 2, g.nx - 1);
     const int k1 = min(k0 + kDense2Z, g.nz);
-    auto ld2 = [&](const float* f, int jj, int kk) { return __ldg(reinterpret_cast<const float2*>(f + g.idx(ic, jj, kk))); };
-    float2 zm = ld2(phi, jc, max(k0 - 1, 0));
-    float2 c = ld2(phi, jc, k0);
+    // row pointers advance by one z-plane per iteration: no index arithmetic inside the loop
+    const int64_t plane = (int64_t)g.nx * g.ny;
+    const int64_t at0 = g.idx(ic, jc, k0);
+    const float* pc = phi + at0;
+    const float* pym = phi + g.idx(ic, jm, k0);
+    const float* pyp = phi + g.idx(ic, jp, k0);
+    const float* pl = phi + g.idx(il, jc, k0);
+    const float* pr = phi + g.idx(ir, jc, k0);
+    const float* pf = F + at0;
+    float* po = out + at0;
+    const bool edge_r = lane == 31 || ic + 2 >= g.nx;
+    auto ld2 = [](const float* q) { return __ldg(reinterpret_cast<const float2*>(q)); };
+    float2 zm = ld2(k0 > 0 ? pc - plane : pc);
+    float2 c = ld2(pc);
     for (int k = k0; k < k1; ++k) {
-        const float2 zp = ld2(phi, jc, min(k + 1, g.nz - 1));
-        const float2 ym = ld2(phi, jm, k), yp = ld2(phi, jp, k);
-        const float2 f = ld2(F, jc, k);
+        const float2 zp = ld2(k + 1 < g.nz ? pc + plane : pc);
+        const float2 ym = ld2(pym), yp = ld2(pyp);
+        const float2 f = ld2(pf);
         float left = __shfl_up_sync(0xffffffffu, c.y, 1), right = __shfl_down_sync(0xffffffffu, c.x, 1);
-        if (lane == 0) left = __ldg(phi + g.idx(il, jc, k));
-        if (lane == 31 || ic + 2 >= g.nx) right = __ldg(phi + g.idx(ir, jc, k));
+        if (lane == 0) left = __ldg(pl);
+        if (edge_r) right = __ldg(pr);
         const float2 u = advance_dense_pair(c, make_float2(left, c.x), make_float2(c.y, right), ym, yp, zm, zp, f, p);
-        if (live) *reinterpret_cast<float2*>(out + g.idx(ic, jc, k)) = u;
+        if (live) *reinterpret_cast<float2*>(po) = u;
         zm = c;
         c = zp;
+        pc += plane; pym += plane; pyp += plane; pl += plane; pr += plane; pf += plane; po += plane;
     }
 }
 
