@@ -491,3 +491,24 @@ def test_full_size_cfg5_reinit_sampled():
         want = orc.reinit(phi_c, Nm, w.dtau, w.dx, w.gamma, iters)
         assert np.array_equal(got[sl][inner], want[inner]), f"crop at {org}"
         assert (Nm[inner] != 0).sum() > 10000
+
+
+@pytest.mark.parametrize("n", [101, 201])
+def test_paper_shaped_grids(n):
+    """the paper's own grid sizes, 101^3 and 201^3, 10 time steps
+    (Tables 1-2).  Its front, F, gamma are not stated, so cfg 1's sphere set-up stands
+    in.  Dimensions that are not multiples of 8 (partial bricks on every high face) nor of 4 (rows not
+    16-byte aligned: the scalar band kernels run, not the TMA ones).  Free-running, both rebuild modes,
+    band export and field compared bit for bit after the last step."""
+    w = inputs.config(1, n=n)
+    steps = 10 if n == 101 else 4      # the oracle sweeps the full 201^3 grid: keep the CPU side in seconds
+    prev, _ = orc.step(w.phi, w.F, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, steps - 1)
+    want, upd = orc.step(prev, w.F, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, 1)
+    upd_prev = orc.step(w.phi, w.F, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, steps - 1)[1]
+    for rebuild in (ls.LS_REBUILD_FULL, ls.LS_REBUILD_INCREMENTAL):
+        with Ctx(w.shape, w.dtype) as ctx:
+            d_phi, d_F = to_dev(w.phi), to_dev(w.F)
+            ls.ls_step(ctx, d_phi, d_F, ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild), steps)
+            assert_band_equal(ctx, prev, w.gamma)      # the band of the last step
+            assert ls.ls_stats(ctx)[0] == upd_prev + upd
+            assert np.array_equal(d_phi.cpu().numpy(), want)
