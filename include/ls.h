@@ -153,6 +153,19 @@ ls_status ls_step(ls_ctx* ctx, void* phi, const void* F, const ls_params* p, int
  * fields, runs n_steps, copies phi back, and synchronises.  The end-to-end entry point. */
 ls_status ls_step_host(ls_ctx* ctx, void* phi_host, const void* F_host, const ls_params* p, int32_t n_steps);
 
+/* m-step batching with snapshot return (the paper keeps m results on the device and
+ * copies them back per host round trip; writing output is ~16 % of its serial run time;
+ * SURVEY.md section 8(f) f-2).  Runs ls_step's Steps 1-3 n_steps times and returns a copy of phi after every
+ * `every`-th step (every >= 1) to HOST memory: host_out receives floor(n_steps / every) fields of
+ * nx*ny*nz elements back to back (pinned memory makes the copies asynchronous; pageable works).
+ * Snapshot k is copied device-to-device into one of two ctx-owned slots on the ctx stream, and from the slot
+ * to the host on a second, ctx-owned stream while the following steps compute (events order the two
+ * streams both ways).  `phi` is updated in place as by ls_step.  Synchronises both streams before it
+ * returns.  HOST out-pointer n_written (may be NULL) = number of snapshots written.
+ * p->chained is honoured for the first step; the remaining steps are chained internally. */
+ls_status ls_step_snapshots(ls_ctx* ctx, void* phi, const void* F, const ls_params* p, int32_t n_steps,
+                            int32_t every, void* host_out, int32_t* n_written);
+
 /* Work counters since ls_create / the last ls_stats_reset: band point updates
  * sum_steps(|T_s| + iters*|N_s|) (dense advance: nx*ny*nz per call), narrow-band steps done, and
  * kernels launched by this ctx.  HOST out-pointers, any may be NULL.  Synchronises. */

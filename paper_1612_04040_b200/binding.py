@@ -26,7 +26,7 @@ KERNEL_KINDS = ("classify", "band", "advance", "reinit", "clamp", "copy")
 SYMBOLS = (
     "ls_status_str", "ls_last_cuda_error", "ls_create", "ls_destroy", "ls_build_band", "ls_band_counts",
     "ls_band_export", "ls_advance", "ls_reinit", "ls_reinit_tol", "ls_step", "ls_step_host", "ls_stats",
-    "ls_stats_reset", "ls_profile_enable", "ls_profile_read", "ls_profile_reset", "ls_selftest_math",
+    "ls_stats_reset", "ls_profile_enable", "ls_profile_read", "ls_profile_reset", "ls_selftest_math", "ls_step_snapshots",
 )
 
 
@@ -76,6 +76,7 @@ def lib() -> C.CDLL:
         L.ls_profile_enable.argtypes = [_P, _I]
         L.ls_profile_read.argtypes = [_P, _I, C.POINTER(_D), C.POINTER(_L)]
         L.ls_profile_reset.argtypes = [_P]
+        L.ls_step_snapshots.argtypes = [_P, _P, _P, C.POINTER(ls_params), _I, _I, _P, C.POINTER(_I)]
         L.ls_selftest_math.argtypes = [_P, C.c_uint64, _L, _D, _D, _D, _D, C.POINTER(_L)]
         for name in SYMBOLS[2:]:
             getattr(L, name).restype = C.c_int
@@ -206,3 +207,12 @@ def ls_selftest_math(seed: int, n: int, dx: float, dt: float, beta: float, gamma
     _ck(lib().ls_selftest_math(_P(cuda_stream), C.c_uint64(seed), n, dx, dt, beta, gamma, C.byref(m)),
         "ls_selftest_math")
     return m.value
+
+
+def ls_step_snapshots(ctx: int, phi, F, p: ls_params, n_steps: int, every: int, host_out) -> int:
+    """-> number of snapshots written to `host_out` (numpy array / CPU tensor of >= n_steps//every fields)."""
+    n = _I()
+    _ck(lib().ls_step_snapshots(_P(ctx), _P(_dev(phi)), _P(_dev(F)), C.byref(p), n_steps, every,
+                                _P(_host(host_out)) if host_out is not None else None, C.byref(n)),
+        "ls_step_snapshots")
+    return n.value

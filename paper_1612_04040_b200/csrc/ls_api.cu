@@ -23,6 +23,9 @@ struct ls_ctx {
     void* scratch;        // one field, second Jacobi buffer (lazy)
     void* dev_phi;        // ls_step_host staging (lazy)
     void* dev_F;
+    void* snap[2];        // ls_step_snapshots: device snapshot slots (lazy)
+    cudaStream_t copy_stream;   // ... and the stream / events of the device-to-host copies (lazy)
+    cudaEvent_t snap_ready[2], snap_free[2];
     unsigned long long* residual;  // device
     ls::Counts* host_counts;       // pinned
     unsigned long long* host_residual;  // pinned
@@ -306,9 +309,14 @@ ls_status ls_destroy(ls_ctx* c) {
     cudaStreamSynchronize(c->stream);
     ls::BandBuffers& bb = c->bb;
     void* dev[] = {bb.tmask, bb.nmask, bb.flagT, bb.flagN, bb.flagNprev, bb.T_ids, bb.N_ids, bb.U_ids, bb.T_pos, bb.N_pos, bb.U_pos,
-                   bb.T_masks, bb.N_masks, bb.partials, bb.counts, c->residual, c->scratch, c->dev_phi, c->dev_F};
+                   bb.T_masks, bb.N_masks, bb.partials, bb.counts, c->residual, c->scratch, c->dev_phi, c->dev_F, c->snap[0], c->snap[1]};
     for (void* p : dev)
         if (p) cudaFree(p);
+    if (c->copy_stream) {
+        cudaStreamSynchronize(c->copy_stream);
+        cudaStreamDestroy(c->copy_stream);
+        for (int i = 0; i < 2; ++i) { cudaEventDestroy(c->snap_ready[i]); cudaEventDestroy(c->snap_free[i]); }
+    }
     if (c->host_counts) cudaFreeHost(c->host_counts);
     if (c->host_residual) cudaFreeHost(c->host_residual);
     for (auto& r : *c->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
@@ -507,6 +515,52 @@ ls_status ls_step_host(ls_ctx* c, void* phi_host, const void* F_host, const ls_p
     LS_CK(cudaMemcpyAsync(phi_host, c->dev_phi, bytes, cudaMemcpyDeviceToHost, c->stream));
     LS_CK(cudaStreamSynchronize(c->stream));
     return LS_OK;
+}
+
+ls_status ls_step_snapshots(ls_ctx* c, void* phi, const void* F, const ls_params* p, int32_t n_steps, int32_t every,
+                            void* host_out, int32_t* n_written) {
+    ls_status st = check_step_args(c, phi, F, p, n_steps);
+    if (st != LS_OK) return st;
+    if (every < 1 || (!host_out && n_steps >= every)) return LS_ERR_ARG;
+    if (n_written) *n_written = 0;
+    if (n_steps == 0) return LS_OK;
+    const size_t bytes = (size_t)c->n * c->elem;
+    if (!c->copy_stream) {
+        LS_CK(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            LS_CK(cudaEventCreateWithFlags(&c->snap_ready[i], cudaEventDisableTiming));
+            LS_CK(cudaEventCreateWithFlags(&c->snap_free[i], cudaEventDisableTiming));
+        }
+    }
+    if ((st = ensure_field(c, &c->snap[0])) != LS_OK) return st;
+    if ((st = ensure_field(c, &c->snap[1])) != LS_OK) return st;
+    ls_params q = *p;
+    int k = 0;   // snapshots taken
+    for (int s = 0; s < n_steps; ++s) {
+        st = c->dtype == LS_F32 ? step_impl<float>(c, (float*)phi, (const float*)F, &q, 1)
+                                : step_impl<double>(c, (double*)phi, (const double*)F, &q, 1);
+        if (st != LS_OK) break;
+        q.chained = 1;   // same buffer, untouched in between
+        if ((s + 1) % every == 0) {
+            const int slot = k & 1;
+            if (k >= 2) LS_CK(cudaStreamWaitEvent(c->stream, c->snap_free[slot], 0));   // its last D2H has drained
+            {
+                ProfScope ps(c, LS_K_COPY);
+                LS_CK(cudaMemcpyAsync(c->snap[slot], phi, bytes, cudaMemcpyDeviceToDevice, c->stream));
+            }
+            LS_CK(cudaEventRecord(c->snap_ready[slot], c->stream));
+            LS_CK(cudaStreamWaitEvent(c->copy_stream, c->snap_ready[slot], 0));
+            LS_CK(cudaMemcpyAsync((char*)host_out + (size_t)k * bytes, c->snap[slot], bytes, cudaMemcpyDeviceToHost,
+                                  c->copy_stream));
+            LS_CK(cudaEventRecord(c->snap_free[slot], c->copy_stream));
+            ++k;
+        }
+    }
+    cudaError_t e1 = cudaStreamSynchronize(c->stream), e2 = cudaStreamSynchronize(c->copy_stream);
+    if (e1 != cudaSuccess) return cuda_fail(e1, "ls_step_snapshots: cudaStreamSynchronize");
+    if (e2 != cudaSuccess) return cuda_fail(e2, "ls_step_snapshots: cudaStreamSynchronize(copy)");
+    if (n_written) *n_written = k;
+    return st;
 }
 
 ls_status ls_stats(ls_ctx* c, int64_t* point_updates, int64_t* steps, int64_t* kernel_launches) {

@@ -512,3 +512,27 @@ def test_paper_shaped_grids(n):
             assert_band_equal(ctx, prev, w.gamma)      # the band of the last step
             assert ls.ls_stats(ctx)[0] == upd_prev + upd
             assert np.array_equal(d_phi.cpu().numpy(), want)
+
+
+def test_step_snapshots_match_oracle_trajectory():
+    """ls_step_snapshots (m-step batching, f-2): every 2nd of 7 steps returned to pinned host memory while
+    the next steps compute; each snapshot equals the oracle's trajectory bit for bit, the final field equals
+    the plain ls_step result, and a chained continuation still matches."""
+    w = inputs.config(3, n=64)
+    traj, cur = [], w.phi
+    for s in range(9):
+        cur, _ = orc.step(cur, w.F, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, 1)
+        traj.append(cur)
+    for rebuild in (ls.LS_REBUILD_FULL, ls.LS_REBUILD_INCREMENTAL):
+        host = torch.empty((3,) + w.shape, dtype=torch.float32).pin_memory()
+        with Ctx(w.shape, w.dtype) as ctx:
+            d_phi, d_F = to_dev(w.phi), to_dev(w.F)
+            p = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild)
+            assert ls.ls_step_snapshots(ctx, d_phi, d_F, p, 7, 2, host) == 3
+            for k in range(3):
+                assert np.array_equal(host[k].numpy(), traj[2 * k + 1]), f"snapshot {k}"
+            assert np.array_equal(d_phi.cpu().numpy(), traj[6])
+            p1 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild, 1)
+            assert ls.ls_step_snapshots(ctx, d_phi, d_F, p1, 2, 5, host) == 0     # fewer steps than `every`
+            assert np.array_equal(d_phi.cpu().numpy(), traj[8])
+            assert ls.ls_stats(ctx)[1] == 9
