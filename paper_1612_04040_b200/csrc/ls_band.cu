@@ -4,11 +4,13 @@
 // Kernels
 //   k_classify        whole-grid sweep, 32x8x8 points per CTA, 128-bit coalesced loads;
 //                     T bits are assembled into brick mask words with warp REDUX (no atomics).
-//   k_dilate          N words = T | shifted T | neighbour-brick faces, one thread per (brick, z-word).
+//   k_dilate          N words = T | shifted T | neighbour-brick faces; one thread per brick, gated by the 7 flag
+//                     bytes of the brick and its face neighbours; also counts |T| and |N|.
 //   k_count / k_scan_partials / k_scatter
 //                     ordered stream compaction of the brick flags by a two-level prefix sum, so the
 //                     lists are ascending in brick id whatever the CTA scheduling (R20).
-//   k_finalize        adds |T| + iters*|N| to the work counter.
+//   k_finalize        folds the point counters, adds |T| + iters*|N| to the work counter.
+//   k_gather_masks    list-ordered mask copies for ls_band_export (T: snapshot per build, N: on demand).
 // Data: per-brick byte flags (nbricks B) and dense mask words (64 B per brick, written only for
 // non-empty bricks) live in the ctx; the compacted lists are what the stencil kernels iterate.
 #include "ls_internal.h"

@@ -5,11 +5,12 @@
 //                        x-fastest field into shared memory, plus the brick's 64-byte
 //                        mask (and, for Advance, the 8^3 box of F), all completing on one mbarrier;
 //                        kStages bricks are in flight per CTA
-//   consumers (8 warps)  wait on the mbarrier; replicate edge values into out-of-domain halo cells
+//   consumers (4 warps)  wait on the mbarrier; replicate edge values into out-of-domain halo cells
 //                        (R3; TMA zero-fills them); compact the brick's active points into a list with
-//                        ballot/popc ranks so warps run full; evaluate eq. 3-8 / eq. 12-13 once per
-//                        active point from the tile; write results back into the tile; store whole
-//                        32-byte rows with 128-bit stores.
+//                        popc / REDUX ranks so warps run full; evaluate eq. 3-8 / eq. 12-13 for two points
+//                        per lane (packed fp32 arithmetic) from the tile into an 8^3 out-brick (Jacobi);
+//                        store whole 32-byte rows with 128-bit stores, merging out-brick and tile values.
+//                        Two CTA barriers per brick (list complete; out-brick complete).
 // The arithmetic is that of ls_math.cuh (IEEE, no FMA contraction): results are bit-identical to the
 // scalar kernels of ls_stencil.cu, which remain the path for grids TMA cannot address
 // (nx*sizeof(T) not a multiple of 16, or unaligned fields).
