@@ -9,7 +9,7 @@
 //   k_count / k_scan_partials / k_scatter
 //                     ordered stream compaction of the brick flags by a two-level prefix sum, so the
 //                     lists are ascending in brick id whatever the CTA scheduling (R20).
-//   k_finalize        folds the point counters, adds |T| + iters*|N| to the work counter.
+//                     (k_scan_partials also folds the point counters and adds |T| + iters*|N| to the work counter)
 //   k_gather_masks    list-ordered mask copies for ls_band_export (T: snapshot per build, N: on demand).
 // Data: per-brick byte flags (nbricks B) and dense mask words (64 B per brick, written only for
 // non-empty bricks) live in the ctx; the compacted lists are what the stencil kernels iterate.
@@ -210,7 +210,7 @@ __global__ void __launch_bounds__(kScanThreads) k_count(const uint8_t* __restric
 
 // Exclusive scan of the per-CTA counts of each list, in place; totals go to Counts.  One CTA.
 __global__ void __launch_bounds__(1024) k_scan_partials(int32_t* __restrict__ partials, int npartials,
-                                                         Counts* __restrict__ counts) {
+                                                         Counts* __restrict__ counts, int iters, int count_step) {
     __shared__ int wsum[32];
     __shared__ int carry_s;
     for (int l = 0; l < 3; ++l) {
@@ -251,6 +251,16 @@ __global__ void __launch_bounds__(1024) k_scan_partials(int32_t* __restrict__ pa
             if (l == 2) counts->nU = carry_s;
         }
         __syncthreads();
+    }
+    if (threadIdx.x == 0) {   // fold the point counters of this build (k_dilate has finished: stream order)
+        counts->nT_pts = counts->acc_T;
+        counts->nN_pts = counts->acc_N;
+        counts->acc_T = 0;
+        counts->acc_N = 0;
+        if (count_step) {
+            counts->updates += counts->nT_pts + (unsigned long long)iters * counts->nN_pts;
+            counts->steps += 1;
+        }
     }
 }
 
@@ -304,17 +314,6 @@ __global__ void __launch_bounds__(256) k_gather_masks(const int32_t* __restrict_
         out[t] = dense[(int64_t)ids[t >> 3] * 8 + (t & 7)];
 }
 
-__global__ void k_finalize(Counts* counts, int iters, int count_step) {
-    counts->nT_pts = counts->acc_T;
-    counts->nN_pts = counts->acc_N;
-    counts->acc_T = 0;
-    counts->acc_N = 0;
-    if (count_step) {
-        counts->updates += counts->nT_pts + (unsigned long long)iters * counts->nN_pts;
-        counts->steps += 1;
-    }
-}
-
 }  // namespace
 
 template <typename T>
@@ -333,13 +332,12 @@ void launch_dilate_compact(const Geom& g, const BandBuffers& bb, int iters, bool
                            int64_t* launches) {
     k_dilate<<<(unsigned)((g.nbricks + 255) / 256), 256, 0, s>>>(g, bb.tmask, bb.flagT, bb.nmask, bb.flagN, bb.counts);
     k_count<<<bb.npartials, kScanThreads, 0, s>>>(bb.flagT, bb.flagN, bb.flagNprev, bb.partials, bb.npartials);
-    k_scan_partials<<<1, 1024, 0, s>>>(bb.partials, bb.npartials, bb.counts);
+    k_scan_partials<<<1, 1024, 0, s>>>(bb.partials, bb.npartials, bb.counts, iters, count_step ? 1 : 0);
     k_scatter<<<bb.npartials, kScanThreads, 0, s>>>(bb.flagT, bb.flagN, bb.flagNprev, bb.partials, bb.npartials, bb, g);
-    k_finalize<<<1, 1, 0, s>>>(bb.counts, iters, count_step ? 1 : 0);
     // Snapshot of the T masks in list order: the last reinit sweep of an incremental step overwrites the
     // dense T masks with those of phi^{n+1}, while ls_band_export reports the band of phi^n.
     k_gather_masks<<<sm_count() * 2, 256, 0, s>>>(bb.T_ids, &bb.counts->nT, bb.tmask, bb.T_masks);
-    if (launches) *launches += 6;
+    if (launches) *launches += 5;
 }
 
 void launch_gather_masks(const BandBuffers& bb, cudaStream_t s, int64_t* launches) {

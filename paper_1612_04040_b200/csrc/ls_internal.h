@@ -26,7 +26,7 @@ struct Counts {
     int32_t nU;            // bricks in the U list (N of this step  ∪  N of the previous step)
     int32_t pad;
     unsigned long long nT_pts, nN_pts;  // |T|, |N|
-    unsigned long long acc_T, acc_N;    // accumulators of the build in flight (k_dilate), folded by k_finalize
+    unsigned long long acc_T, acc_N;    // accumulators of the build in flight (k_dilate), folded by k_scan_partials
     unsigned long long updates;         // sum over steps of |T| + iters*|N|
     unsigned long long steps;
 };
