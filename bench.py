@@ -317,7 +317,7 @@ def run_ours(args):
                 "frac_of_8TBps_nominal": (ach / 8000.0) if ach else None}
     cpu = None
     if not args.no_cpu_baseline:
-        g, sps, threads, sample = time_oracle(w, 2, 1)
+        g, sps, threads, sample = time_oracle(w, 20, 1)   # ~10 s of CPU work on the GPU box (0.44 s per slab step)
         cpu = {"value": g, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample, "s_per_step": sps}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
