@@ -18,7 +18,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 SO = PKG / "libls.so"
-SOURCES = ["ls_band.cu", "ls_stencil.cu", "ls_tma.cu", "ls_api.cu"]
+SOURCES = ["ls_band.cu", "ls_stencil.cu", "ls_tile.cu", "ls_api.cu"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-fmad=false",
     "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math,-Wall", "-cudart", "static", "-shared",

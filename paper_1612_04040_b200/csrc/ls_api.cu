@@ -1,6 +1,6 @@
 // ls_api.cu — the C ABI of include/ls.h: context, argument checks, and the host driver of the
 // Step 1-3 loop on one stream.  Every step of the path runs in the kernels of
-// ls_band.cu / ls_stencil.cu; this file only sequences launches.  There is no CPU fallback.
+// ls_band.cu / ls_tile.cu / ls_stencil.cu; this file only sequences launches.  There is no CPU fallback.
 #include <cmath>
 #include <cstddef>
 #include <cstdio>
@@ -12,8 +12,6 @@
 
 #include "../../include/ls.h"
 #include "ls_internal.h"
-
-namespace ls { int scan_tile(); }
 
 struct ls_ctx {
     ls::Geom g;
@@ -37,7 +35,8 @@ struct ls_ctx {
     // chained stepping (ls_params::chained): what the last ls_step left behind
     const void* chain_phi;   // phi buffer the ctx state is consistent with (null: none)
     double chain_gamma;
-    bool chain_have_T;       // tmask / flagT already hold the T masks of the current phi
+    bool chain_have_T;       // tmask[tb ^ 1] holds the T masks of the current phi (emitted by the last sweep)
+    bool flip;               // list walking direction of the next band launch
     // per-kernel device timing (ls_profile_*)
     bool prof_on;
     struct ProfRec { int kind; cudaEvent_t a, b; };
@@ -116,6 +115,7 @@ ls::StencilParams<T> make_params(double dx, double dt, double beta, double gamma
     ls::StencilParams<T> p;
     const T dxT = (T)dx;
     p.inv_dx = T(1) / dxT;
+    p.half_inv_dx = p.inv_dx * T(0.5);
     p.dx2 = dxT * dxT;
     p.dt = (T)dt;
     p.beta = (T)beta;
@@ -139,7 +139,21 @@ bool bad_band_params(double dx, double beta, double gamma) {
     return !(beta > 0 && beta < gamma);
 }
 
-ls_status build_band_impl(ls_ctx* c, const void* phi, double gamma, int iters, bool count_step, bool classify) {
+// One band launch: the tile kernels where they can address the grid, else the scalar kernels.
+template <typename T>
+void band_launch(ls_ctx* c, const T* src, const T* F, T* dst, const ls::StencilParams<T>& p, ls::BandOp op) {
+    op.reverse = c->flip;
+    c->flip = !c->flip;
+    if (!op.copy && ls::tile_usable<T>(c->g, src, F, dst) &&
+        ls::launch_band_tile<T>(src, F, dst, c->g, p, c->bb, op, c->stream, &c->launches))
+        return;
+    ls::launch_band_scalar<T>(src, F, dst, c->g, p, c->bb, op, c->stream, &c->launches);
+}
+
+// Step 1.  classify: scan the whole grid for T (else tmask[tb] already holds T of phi, emitted by the last
+// sweep of the previous step); incremental: candidates from the previous band only.
+ls_status build_band_impl(ls_ctx* c, const void* phi, double gamma, int iters, bool count_step, bool classify,
+                          bool incremental) {
     if (classify) {
         ProfScope ps(c, LS_K_CLASSIFY);
         if (c->dtype == LS_F32)
@@ -149,13 +163,20 @@ ls_status build_band_impl(ls_ctx* c, const void* phi, double gamma, int iters, b
     }
     {
         ProfScope ps(c, LS_K_BAND);
-        ls::launch_dilate_compact(c->g, c->bb, iters, count_step, c->stream, &c->launches);
+        ls::launch_build_lists(c->g, c->bb, incremental, iters, count_step, c->stream, &c->launches);
     }
     LS_CK_LAUNCH();
     c->band_valid = true;
     return LS_OK;
 }
 
+// Steps 1-3, n_steps times.  Two Jacobi buffers: the caller's phi and the ctx scratch field S.
+//   Advance phi -> S, sweeps S -> phi -> S ..., the last one landing in phi (even `iters`: a band copy).
+// Only item cells are written, so the buffers must agree wherever a later launch reads a halo.  Invariant at
+// the start of a chained step n: S == phi^n except on the item cells of the band of step n-1 (they hold the
+// next-to-last iterate).  Since T^n is a subset of N^{n-1}, Advance of step n walks the items of
+// the PREVIOUS band: T cells get eq. 8, the other cells are copied — which repairs S exactly where it is stale.
+// The first step of an unchained call starts from S = phi (one whole-field copy) and walks its own band.
 template <typename T>
 ls_status step_impl(ls_ctx* c, T* phi, const T* F, const ls_params* p, int n_steps) {
     ls_status st = ensure_field(c, &c->scratch);
@@ -165,46 +186,73 @@ ls_status step_impl(ls_ctx* c, T* phi, const T* F, const ls_params* p, int n_ste
     const ls::StencilParams<T> rei = make_params<T>(p->dx, p->dtau, p->beta, p->gamma);
     const T gammaT = (T)p->gamma;
     cudaStream_t s = c->stream;
-    // chained: the ctx state (S consistent with phi off the band, flagNprev = N of the last step,
-    // phi clamped everywhere) carries over from the previous call.
+    const bool incremental = p->rebuild == LS_REBUILD_INCREMENTAL;
     const bool chained = p->chained && c->chain_phi == (const void*)phi && c->chain_gamma == p->gamma;
-    bool have_T = chained && c->chain_have_T && p->rebuild == LS_REBUILD_INCREMENTAL;
+    bool have_T = chained && c->chain_have_T && incremental;
     c->chain_phi = nullptr;   // re-established only when the whole call was enqueued
     if (!chained) {
-        // Both Jacobi buffers must agree off the band: start from a full copy, and forget the previous
-        // call's N (the U list is then just N in the first step).
         ProfScope ps(c, LS_K_COPY);
         LS_CK(cudaMemcpyAsync(S, phi, (size_t)c->n * sizeof(T), cudaMemcpyDeviceToDevice, s));
-        LS_CK(cudaMemsetAsync(c->bb.flagNprev, 0, (size_t)c->g.nbricks, s));
     }
     for (int step = 0; step < n_steps; ++step) {
-        st = build_band_impl(c, phi, p->gamma, p->iters, true, !have_T);   // Step 1
-        if (st != LS_OK) return st;
-        {
-            ProfScope ps(c, LS_K_ADVANCE);
-            ls::launch_advance_band<T>(phi, F, S, c->g, adv, c->bb, false, s, &c->launches);   // Step 2: phi -> S
+        const bool have_prev = chained || step > 0;   // S is stale on the previous band's items
+        if (have_T) {   // the last sweep left T of phi^n in the other T buffer, valid on the quads of the band it walked
+            c->bb.tb ^= 1;
+            c->bb.tvalid_all = false;
         }
-        // T masks of phi^{n+1} come out of the last sweep (the one that writes phi): odd iters only
-        const bool emit = p->rebuild == LS_REBUILD_INCREMENTAL && (p->iters & 1);
+        ls::BandOp a;
+        a.advance = true;
+        if (have_prev) {
+            // Step 2 first (it needs T^n and the PREVIOUS band's lists), then Step 1 for the sweeps
+            if (!have_T) {
+                ProfScope ps(c, LS_K_CLASSIFY);
+                ls::launch_classify<T>(phi, c->g, gammaT, c->bb, s, &c->launches);
+            }
+            a.list = c->bb.lb;
+            {
+                ProfScope ps(c, LS_K_ADVANCE);
+                band_launch<T>(c, phi, F, S, adv, a);
+            }
+            st = build_band_impl(c, phi, p->gamma, p->iters, true, false, have_T);
+            if (st != LS_OK) return st;
+        } else {
+            st = build_band_impl(c, phi, p->gamma, p->iters, true, true, false);   // Step 1 (whole grid)
+            if (st != LS_OK) return st;
+            a.list = c->bb.lb;
+            ProfScope ps(c, LS_K_ADVANCE);
+            band_launch<T>(c, phi, F, S, adv, a);                                   // Step 2: phi -> S
+        }
         T* src = S;
         T* dst = phi;
-        for (int it = 0; it < p->iters; ++it) {                             // Step 3
-            const bool last = it == p->iters - 1;
+        bool emitted = false;
+        for (int it = 0; it < p->iters; ++it) {                                     // Step 3
+            const bool last = it == p->iters - 1 && dst == phi;
+            ls::BandOp r;
+            r.sweeps = 1;
+            r.list = c->bb.lb;
+            r.clamp = last;
+            r.emit_T = last && incremental;
+            emitted = emitted || r.emit_T;
             ProfScope ps(c, LS_K_REINIT);
-            ls::launch_reinit_band<T>(src, dst, c->g, rei, c->bb, last, nullptr, emit && last, s, &c->launches);
+            band_launch<T>(c, src, (const T*)nullptr, dst, rei, r);
             T* t = src; src = dst; dst = t;
         }
         if (src != phi) {  // even iters: the result sits in S
+            ls::BandOp r;
+            r.copy = true;
+            r.list = c->bb.lb;
+            r.clamp = true;
+            r.emit_T = incremental;
+            emitted = r.emit_T;
             ProfScope ps(c, LS_K_CLAMP);
-            ls::launch_copy_clamp_band<T>(S, phi, c->g, gammaT, c->bb, s, &c->launches);
+            band_launch<T>(c, S, (const T*)nullptr, phi, rei, r);
         }
-        if (step == 0 && !chained) {  // eq. 10 at every point (R14); afterwards points off N already hold +-gamma
+        if (!have_prev) {  // eq. 10 at every point (R14); afterwards points off N already hold +-gamma
             ProfScope ps(c, LS_K_CLAMP);
             ls::launch_clamp_all<T>(phi, S, c->n, gammaT, s, &c->launches);
         }
         LS_CK_LAUNCH();
-        have_T = emit;
-        uint8_t* t = c->bb.flagN; c->bb.flagN = c->bb.flagNprev; c->bb.flagNprev = t;
+        have_T = emitted;
     }
     c->chain_phi = phi;
     c->chain_gamma = p->gamma;
@@ -249,15 +297,14 @@ ls_status ls_create(int32_t nx, int32_t ny, int32_t nz, ls_dtype dtype, void* cu
     if (dtype != LS_F32 && dtype != LS_F64) return LS_ERR_DTYPE;
     const int64_t NBx = (nx + 7) / 8, NBy = (ny + 7) / 8, NBz = (nz + 7) / 8;
     const int64_t nbricks = NBx * NBy * NBz;
-    if (nbricks > (int64_t)1 << 27) return LS_ERR_DIM;   // brick ids, tile counts and 8*id stay in range
+    const int64_t NQx = (NBx + 3) / 4, nquads = NQx * NBy * NBz;
+    if (nbricks > (int64_t)1 << 27) return LS_ERR_DIM;   // brick ids, quad ids and 32*quad stay in range
     int ndev = 0;
     LS_CK(cudaGetDeviceCount(&ndev));
     ls_ctx* c = new (std::nothrow) ls_ctx();
     if (!c) return LS_ERR_ALLOC;
     std::memset(c, 0, sizeof *c);
-    auto bits = [](int64_t n) { int b = 0; while (((int64_t)1 << b) < n) ++b; return b; };   // ceil(log2 n)
-    const int wx = bits(NBx), wy = bits(NBy);   // wx + wy + bits(NBz) <= 27 + 3
-    c->g = ls::Geom{nx, ny, nz, (int)NBx, (int)NBy, (int)NBz, (int)nbricks, (1 << wx) - 1, (1 << wy) - 1, wx, wx + wy};
+    c->g = ls::Geom{nx, ny, nz, (int)NBx, (int)NBy, (int)NBz, (int)NQx, (int)nbricks, (int)nquads};
     c->dtype = dtype;
     c->stream = (cudaStream_t)cuda_stream;
     c->elem = dtype == LS_F32 ? 4 : 8;
@@ -265,30 +312,25 @@ ls_status ls_create(int32_t nx, int32_t ny, int32_t nz, ls_dtype dtype, void* cu
     c->prof_recs = new (std::nothrow) std::vector<ls_ctx::ProfRec>();
     c->prof_pool = new (std::nothrow) std::vector<cudaEvent_t>();
     if (!c->prof_recs || !c->prof_pool) { delete c->prof_recs; delete c->prof_pool; delete c; return LS_ERR_ALLOC; }
-    const int tile = ls::scan_tile();
-    const int64_t padded = (nbricks + tile - 1) / tile * tile;
     ls::BandBuffers& bb = c->bb;
-    bb.npartials = (int)(padded / tile);
+    bb.compact_grid = (int)std::min<int64_t>(ls::sm_count(), std::max<int64_t>(1, (nquads + 16383) / 16384));
     cudaError_t e = cudaSuccess;
     auto alloc = [&](void** p, size_t bytes, bool zero) {
         if (e != cudaSuccess) return;
         e = cudaMalloc(p, bytes);
         if (e == cudaSuccess && zero) e = cudaMemsetAsync(*p, 0, bytes, c->stream);
     };
-    alloc((void**)&bb.tmask, (size_t)nbricks * 64, false);
-    alloc((void**)&bb.nmask, (size_t)nbricks * 64, false);
-    alloc((void**)&bb.flagT, (size_t)padded, true);
-    alloc((void**)&bb.flagN, (size_t)padded, true);
-    alloc((void**)&bb.flagNprev, (size_t)padded, true);
-    alloc((void**)&bb.T_ids, (size_t)nbricks * 4, false);
-    alloc((void**)&bb.N_ids, (size_t)nbricks * 4, false);
-    alloc((void**)&bb.U_ids, (size_t)nbricks * 4, false);
-    alloc((void**)&bb.T_pos, (size_t)nbricks * 4, false);
-    alloc((void**)&bb.N_pos, (size_t)nbricks * 4, false);
-    alloc((void**)&bb.U_pos, (size_t)nbricks * 4, false);
-    alloc((void**)&bb.T_masks, (size_t)nbricks * 64, false);
-    alloc((void**)&bb.N_masks, (size_t)nbricks * 64, false);
-    alloc((void**)&bb.partials, (size_t)bb.npartials * 3 * 4, true);
+    const size_t nq = (size_t)nquads;
+    for (int i = 0; i < 2; ++i) {
+        alloc((void**)&bb.tmask[i], nq * 32 * sizeof(uint64_t), false);
+        alloc((void**)&bb.qflagT[i], nq + 16, true);
+        alloc((void**)&bb.qflagN[i], nq + 16, true);          // invariant: 1 exactly at the quads of qlist[i]
+        alloc((void**)&bb.items[i], nq * ls::kItemsPerQuad * sizeof(uint16_t), false);
+        alloc((void**)&bb.qlist[i], nq * sizeof(ls::QuadEntry), false);
+    }
+    alloc((void**)&bb.nmask, nq * 32 * sizeof(uint64_t), true);   // invariant: zero outside the band last built
+    alloc((void**)&bb.qcount, nq * sizeof(int32_t), true);
+    alloc((void**)&bb.partials, 1024 * sizeof(int32_t), true);
     alloc((void**)&bb.counts, sizeof(ls::Counts), true);
     alloc((void**)&c->residual, 8, true);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&c->host_counts, sizeof(ls::Counts));
@@ -308,8 +350,9 @@ ls_status ls_destroy(ls_ctx* c) {
     if (!c) return LS_OK;
     cudaStreamSynchronize(c->stream);
     ls::BandBuffers& bb = c->bb;
-    void* dev[] = {bb.tmask, bb.nmask, bb.flagT, bb.flagN, bb.flagNprev, bb.T_ids, bb.N_ids, bb.U_ids, bb.T_pos, bb.N_pos, bb.U_pos,
-                   bb.T_masks, bb.N_masks, bb.partials, bb.counts, c->residual, c->scratch, c->dev_phi, c->dev_F, c->snap[0], c->snap[1]};
+    void* dev[] = {bb.tmask[0], bb.tmask[1], bb.qflagT[0], bb.qflagT[1], bb.qflagN[0], bb.qflagN[1], bb.items[0], bb.items[1],
+                   bb.qlist[0], bb.qlist[1], bb.nmask, bb.qcount, bb.partials, bb.counts, bb.ex_cnt, bb.T_ids, bb.N_ids,
+                   bb.T_masks, bb.N_masks, c->residual, c->scratch, c->dev_phi, c->dev_F, c->snap[0], c->snap[1]};
     for (void* p : dev)
         if (p) cudaFree(p);
     if (c->copy_stream) {
@@ -332,31 +375,34 @@ ls_status ls_build_band(ls_ctx* c, const void* phi, double dx, double gamma) {
     if (!c || !phi) return LS_ERR_ARG;
     if (!(dx > 0) || !(gamma > 0)) return LS_ERR_ARG;
     c->chain_phi = nullptr;
-    LS_CK(cudaMemsetAsync(c->bb.flagNprev, 0, (size_t)c->g.nbricks, c->stream));
-    return build_band_impl(c, phi, gamma, 0, false, true);
+    return build_band_impl(c, phi, gamma, 0, false, true, false);
 }
 
 ls_status ls_band_counts(ls_ctx* c, int64_t* nT_points, int64_t* nN_points, int32_t* nT_bricks, int32_t* nN_bricks) {
     if (!c) return LS_ERR_ARG;
     if (!c->band_valid) return LS_ERR_STATE;
+    if (nT_bricks || nN_bricks) {   // brick counts are derived from the quad list on demand
+        if (!ls::launch_export(c->g, c->bb, false, c->stream, &c->launches)) return LS_ERR_ALLOC;
+        LS_CK_LAUNCH();
+    }
     LS_CK(cudaMemcpyAsync(c->host_counts, c->bb.counts, sizeof(ls::Counts), cudaMemcpyDeviceToHost, c->stream));
     LS_CK(cudaStreamSynchronize(c->stream));
     if (nT_points) *nT_points = (int64_t)c->host_counts->nT_pts;
     if (nN_points) *nN_points = (int64_t)c->host_counts->nN_pts;
-    if (nT_bricks) *nT_bricks = c->host_counts->nT;
-    if (nN_bricks) *nN_bricks = c->host_counts->nN;
+    if (nT_bricks) *nT_bricks = c->host_counts->nT_bricks;
+    if (nN_bricks) *nN_bricks = c->host_counts->nN_bricks;
     return LS_OK;
 }
 
 ls_status ls_band_export(ls_ctx* c, int32_t* T_ids, uint64_t* T_masks, int32_t* N_ids, uint64_t* N_masks) {
-    int32_t nT = 0, nN = 0;
-    ls_status st = ls_band_counts(c, nullptr, nullptr, &nT, &nN);
-    if (st != LS_OK) return st;
+    if (!c) return LS_ERR_ARG;
+    if (!c->band_valid) return LS_ERR_STATE;
     cudaStream_t s = c->stream;
-    if (N_masks) {   // list-ordered copy of the dense per-brick N masks
-        ls::launch_gather_masks(c->bb, s, &c->launches);
-        LS_CK_LAUNCH();
-    }
+    if (!ls::launch_export(c->g, c->bb, true, s, &c->launches)) return LS_ERR_ALLOC;
+    LS_CK_LAUNCH();
+    LS_CK(cudaMemcpyAsync(c->host_counts, c->bb.counts, sizeof(ls::Counts), cudaMemcpyDeviceToHost, s));
+    LS_CK(cudaStreamSynchronize(s));
+    const int32_t nT = c->host_counts->nT_bricks, nN = c->host_counts->nN_bricks;
     if (T_ids && nT) LS_CK(cudaMemcpyAsync(T_ids, c->bb.T_ids, (size_t)nT * 4, cudaMemcpyDeviceToHost, s));
     if (T_masks && nT) LS_CK(cudaMemcpyAsync(T_masks, c->bb.T_masks, (size_t)nT * 64, cudaMemcpyDeviceToHost, s));
     if (N_ids && nN) LS_CK(cudaMemcpyAsync(N_ids, c->bb.N_ids, (size_t)nN * 4, cudaMemcpyDeviceToHost, s));
@@ -390,12 +436,16 @@ ls_status ls_advance(ls_ctx* c, const void* phi, const void* F, double dt, doubl
         LS_CK(cudaMemcpyAsync(out, phi, (size_t)c->n * c->elem, cudaMemcpyDeviceToDevice, s));
     }
     ProfScope ps(c, LS_K_ADVANCE);
+    ls::BandOp a;
+    a.advance = true;
+    a.list = c->bb.lb;
+    // T of the band last built: emitted masks are valid only on the quads of the band before it
+    a.tgate = c->bb.tvalid_all ? nullptr : c->bb.qflagN[c->bb.lb ^ 1];
     if (c->dtype == LS_F32)
-        ls::launch_advance_band<float>((const float*)phi, (const float*)F, (float*)out, c->g,
-                                       make_params<float>(dx, dt, beta, gamma), c->bb, true, s, &c->launches);
+        band_launch<float>(c, (const float*)phi, (const float*)F, (float*)out, make_params<float>(dx, dt, beta, gamma), a);
     else
-        ls::launch_advance_band<double>((const double*)phi, (const double*)F, (double*)out, c->g,
-                                        make_params<double>(dx, dt, beta, gamma), c->bb, true, s, &c->launches);
+        band_launch<double>(c, (const double*)phi, (const double*)F, (double*)out,
+                            make_params<double>(dx, dt, beta, gamma), a);
     LS_CK_LAUNCH();
     return LS_OK;
 }
@@ -433,8 +483,11 @@ ls_status reinit_impl(ls_ctx* c, T* d, const T* phi_bar, double dtau, double dx,
         if (check) LS_CK(cudaMemsetAsync(c->residual, 0, 8, s));
         {
             ProfScope ps(c, LS_K_REINIT);
-            ls::launch_reinit_band<T>(src, dst, c->g, rei, c->bb, false, check ? c->residual : nullptr, false, s,
-                                      &c->launches);
+            ls::BandOp r;
+            r.sweeps = 1;
+            r.list = c->bb.lb;
+            r.residual = check ? c->residual : nullptr;
+            band_launch<T>(c, src, (const T*)nullptr, dst, rei, r);
         }
         T* t = src; src = dst; dst = t;
         if (check) {
@@ -616,7 +669,7 @@ ls_status ls_selftest_math(void* cuda_stream, uint64_t seed, int64_t n, double d
     const unsigned long long h = out.n[0];
     if (h && getenv("LS_SELFTEST_VERBOSE")) {   // first differing sample: stencils (zm ym xm c xp yp zp) x2, F, scalar / packed results
         std::fprintf(stderr, "ls_selftest_math: %llu results differ; first sample:\n", h);
-        for (int k = 0; k < 26; ++k) {
+        for (int k = 0; k < 32; ++k) {
             unsigned bits;
             std::memcpy(&bits, &out.v[k], 4);
             std::fprintf(stderr, "  [%2d] %.9g (0x%08x)\n", k, out.v[k], bits);

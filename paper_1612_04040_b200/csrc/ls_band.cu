@@ -1,27 +1,24 @@
-// ls_band.cu — Step 1: tubes T (eq. 6) and N (eq. 11) as
-// ascending lists of 8^3 bricks with 512-bit masks.
+// ls_band.cu — Step 1: tubes T (eq. 6) and N (eq. 11).
 //
 // Kernels
-//   k_classify        whole-grid sweep, 32x8x8 points per CTA, 128-bit coalesced loads;
-//                     T bits are assembled into brick mask words with warp REDUX (no atomics).
-//   k_dilate          N words = T | shifted T | neighbour-brick faces; one thread per brick, gated by the 7 flag
-//                     bytes of the brick and its face neighbours; also counts |T| and |N|.
-//   k_count / k_scan_partials / k_scatter
-//                     ordered stream compaction of the brick flags by a two-level prefix sum, so the
-//                     lists are ascending in brick id whatever the CTA scheduling (R20).
-//                     (k_scan_partials also folds the point counters and adds |T| + iters*|N| to the work counter)
-//   k_gather_masks    list-ordered mask copies for ls_band_export (T: snapshot per build, N: on demand).
-// Data: per-brick byte flags (nbricks B) and dense mask words (64 B per brick, written only for
-// non-empty bricks) live in the ctx; the compacted lists are what the stencil kernels iterate.
+//   k_classify        whole-grid sweep, one CTA per quad (32x8x8 points), 128-bit coalesced
+//                     loads; T bits are assembled into brick mask words with warp REDUX (no atomics).
+//   k_dilate_items    one WARP per candidate quad: lane (j, lz) builds N word lz of brick j from its own T
+//                     word, its neighbours' words by shuffle, and the facing bit planes of the six
+//                     neighbour quads (eq. 11, R6); then the quad's item list (ls_internal.h) by a warp
+//                     scan.  Candidates: every quad (first build, LS_REBUILD_FULL) or, incrementally, the
+//                     quads of the previous band and their face neighbours (T^{n+1} is a subset of N^n,
+//                     PAPER.md:65) — O(band), not O(grid).  Counts |T| and |N| (integer adds commute).
+//   k_compact         ordered stream compaction of the quad flags into the quad list: per-CTA counts, one
+//                     grid barrier, exclusive scan, scatter — ascending quad id whatever the scheduling
+//                     (R20: no atomics-order dependence).  Also folds the point counters.
+//   k_export_*        brick lists in ls.h's format (ascending brick id + 8 mask words per brick) for
+//                     ls_band_counts / ls_band_export, derived from the quad list on demand.
 #include "ls_internal.h"
 
 namespace ls {
 
 namespace {
-
-constexpr int kScanThreads = 256;
-constexpr int kItemsPerThread = 16;
-constexpr int kScanTile = kScanThreads * kItemsPerThread;  // 4096 bricks per CTA
 
 constexpr uint64_t COL0 = 0x0101010101010101ull;  // lx == 0 in every row
 constexpr uint64_t COL7 = 0x8080808080808080ull;  // lx == 7 in every row
@@ -30,22 +27,22 @@ template <typename T> __device__ __forceinline__ T absval(T v);
 template <> __device__ __forceinline__ float absval<float>(float v) { return fabsf(v); }
 template <> __device__ __forceinline__ double absval<double>(double v) { return fabs(v); }
 
-// One CTA = 32(x) x 8(y) x 8(z) points = 4 bricks in a row.  Warp w owns z-layer w; lane l owns the
-// 4 consecutive x cells x4 = l&7 of row y = (l>>3) + 4h, h = 0,1.  With VEC the 4 cells are one
-// 128-bit load and a warp load covers 4 full 128-byte lines.
+// One CTA = one quad = 32(x) x 8(y) x 8(z) points.  Warp w owns z-layer w; lane l owns the 4 consecutive
+// x cells x4 = l&7 of row y = (l>>3) + 4h, h = 0,1.  With VEC the 4 cells are one 128-bit load and a warp
+// load covers 4 full 128-byte lines.  Writes all 32 mask words of the quad (zeros included) and its flag.
 template <typename T, bool VEC>
-__global__ void __launch_bounds__(256) k_classify(const T* __restrict__ phi, Geom g, int ntx, T gamma,
-                                                  uint64_t* __restrict__ tmask, uint8_t* __restrict__ flagT) {
-    __shared__ uint32_t half_words[8][4][2];  // [lz][brick in tile][low/high 32 bits]
-    const int tile = blockIdx.x;
-    const int tx = tile % ntx;
-    const int by = (tile / ntx) % g.NBy;
-    const int bz = tile / (ntx * g.NBy);
+__global__ void __launch_bounds__(256) k_classify(const T* __restrict__ phi, Geom g, T gamma,
+                                                  uint64_t* __restrict__ tmask, uint8_t* __restrict__ qflagT) {
+    __shared__ uint32_t half_words[8][4][2];  // [lz][brick in quad][low/high 32 bits]
+    const int quad = blockIdx.x;
+    const int qx = quad % g.NQx;
+    const int by = (quad / g.NQx) % g.NBy;
+    const int bz = quad / (g.NQx * g.NBy);
     const int lane = threadIdx.x & 31, lz = threadIdx.x >> 5;
     const int k = bz * 8 + lz;
     const int x4 = lane & 7;
-    const int i0 = tx * 32 + x4 * 4;
-    const int q = x4 >> 1;                                  // brick of the tile this lane feeds
+    const int i0 = qx * 32 + x4 * 4;
+    const int q = x4 >> 1;                                  // brick of the quad this lane feeds
     const unsigned group = 0x03030303u << (2 * q);          // the 8 lanes feeding the same 32-bit half
 
 #pragma unroll
@@ -82,19 +79,14 @@ __global__ void __launch_bounds__(256) k_classify(const T* __restrict__ phi, Geo
         const int qq = threadIdx.x >> 3, z = threadIdx.x & 7;
         const uint64_t word = (uint64_t)half_words[z][qq][0] | ((uint64_t)half_words[z][qq][1] << 32);
         const unsigned nz_lanes = __ballot_sync(0xffffffffu, word != 0);
-        const bool brick_any = ((nz_lanes >> (qq * 8)) & 0xffu) != 0;
-        const int bx = tx * 4 + qq;
-        if (bx < g.NBx) {
-            const int b = (bz * g.NBy + by) * g.NBx + bx;
-            if (brick_any) tmask[(int64_t)b * 8 + z] = word;
-            if (z == 0) flagT[b] = brick_any ? 1 : 0;
-        }
+        tmask[(int64_t)quad * 32 + threadIdx.x] = word;
+        if (threadIdx.x == 0) qflagT[quad] = nz_lanes ? 1 : 0;
     }
 }
 
 // Bits of the cells of brick (bx,by,bz), word lz, that lie inside the domain.
 __device__ __forceinline__ uint64_t domain_word(const Geom& g, int bx, int by, int bz, int lz) {
-    if (bz * 8 + lz >= g.nz) return 0;
+    if (bx >= g.NBx || bz * 8 + lz >= g.nz) return 0;
     const int vx = min(8, g.nx - bx * 8), vy = min(8, g.ny - by * 8);
     const uint64_t rowbits = (1ull << vx) - 1ull;            // vx <= 8
     uint64_t w = rowbits * COL0;                             // replicate into all 8 rows
@@ -102,157 +94,275 @@ __device__ __forceinline__ uint64_t domain_word(const Geom& g, int bx, int by, i
     return w;
 }
 
-// eq. 11 (R6): N = T or any in-domain face neighbour in T.  One thread per brick: 7 flag bytes decide
-// whether the brick can hold N points at all (3 % of the bricks of cfg 4 can); only those touch masks.
-// Also counts |T| and |N| into the accumulators of Counts (integer adds commute: order independent).
-__global__ void __launch_bounds__(256) k_dilate(Geom g, const uint64_t* __restrict__ tmask,
-                                                const uint8_t* __restrict__ flagT, uint64_t* __restrict__ nmask,
-                                                uint8_t* __restrict__ flagN, Counts* __restrict__ counts) {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    unsigned ptsT = 0, ptsN = 0;
-    if (b < g.nbricks) {
-        const int bx = b % g.NBx, by = (b / g.NBx) % g.NBy, bz = b / (g.NBx * g.NBy);
-        const int sx = 1, sy = g.NBx, sz = g.NBx * g.NBy;
-        const bool self = flagT[b] != 0;
-        const bool xm = bx > 0 && flagT[b - sx], xp = bx < g.NBx - 1 && flagT[b + sx];
-        const bool ym = by > 0 && flagT[b - sy], yp = by < g.NBy - 1 && flagT[b + sy];
-        const bool zm = bz > 0 && flagT[b - sz], zp = bz < g.NBz - 1 && flagT[b + sz];
-        bool any = false;
-        if (self | xm | xp | ym | yp | zm | zp) {
-            uint64_t own[8];
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                ulonglong2 v = make_ulonglong2(0ull, 0ull);
-                if (self) v = reinterpret_cast<const ulonglong2*>(tmask + (int64_t)b * 8)[i];
-                own[2 * i] = v.x;
-                own[2 * i + 1] = v.y;
+struct DilateArgs {
+    const uint64_t* tmask;     // T masks to dilate
+    const uint8_t* qflagT;
+    const uint8_t* tgate;      // null: T valid for every quad; else T valid only where tgate != 0 (= qflagN of the previous band)
+    const uint8_t* prevN;      // qflagN of the previous band (list buffer lb)
+    const QuadEntry* prevList; // its quad list ...
+    const int32_t* prevCount;  // ... and length
+    const QuadEntry* staleList;// quad list last stored in the buffer being rebuilt (its flags must be cleared) ...
+    const int32_t* staleCount; // ... and length
+    uint64_t* nmask;
+    uint8_t* qflagN;           // out: flags of the band being built
+    int32_t* qcount;           // out: items per quad
+    uint16_t* items;           // out: item lists
+    Counts* counts;
+};
+
+constexpr int kDilateWarps = 4;
+
+// Which quad does candidate `wid` stand for?  -1: none (out of range, or another candidate owns the quad).
+// Incremental candidates: (entry e of the previous list, direction d = self, -x, +x, -y, +y, -z, +z), then the
+// quads of the stale list.  A quad is processed by exactly one candidate: the first (e, d) in direction order
+// that reaches it; stale entries only if no (e, d) reaches them.
+__device__ __forceinline__ int candidate_quad(const Geom& g, const DilateArgs& a, int64_t wid, int nprev, int nstale) {
+    const int sxq = 1, syq = g.NQx, szq = g.NQx * g.NBy;
+    const int dq[7] = {0, -sxq, sxq, -syq, syq, -szq, szq};
+    if (wid < (int64_t)nprev * 7) {
+        const int e = (int)(wid / 7), d = (int)(wid % 7);
+        const int sq = a.prevList[e].quad;
+        const int qx = sq % g.NQx, by = (sq / g.NQx) % g.NBy, bz = sq / szq;
+        const bool inside = d == 0 || (d == 1 && qx > 0) || (d == 2 && qx < g.NQx - 1) || (d == 3 && by > 0) ||
+                            (d == 4 && by < g.NBy - 1) || (d == 5 && bz > 0) || (d == 6 && bz < g.NBz - 1);
+        if (!inside) return -1;
+        const int c = sq + dq[d];
+        if (d != 0) {
+            if (a.prevN[c]) return -1;   // reached by its own (e', self)
+            const int cx = c % g.NQx, cy = (c / g.NQx) % g.NBy, cz = c / szq;
+            for (int dd = 1; dd < d; ++dd) {   // an earlier direction dd reaches c from the source c - dq[dd]
+                const bool in2 = (dd == 1 && cx < g.NQx - 1) || (dd == 2 && cx > 0) || (dd == 3 && cy < g.NBy - 1) ||
+                                 (dd == 4 && cy > 0) || (dd == 5 && cz < g.NBz - 1) || (dd == 6 && cz > 0);
+                if (in2 && a.prevN[c - dq[dd]]) return -1;
             }
-            const uint64_t below = zm ? tmask[(int64_t)(b - sz) * 8 + 7] : 0ull;
-            const uint64_t above = zp ? tmask[(int64_t)(b + sz) * 8 + 0] : 0ull;
-            const uint64_t* txm = tmask + (int64_t)(b - sx) * 8;
-            const uint64_t* txp = tmask + (int64_t)(b + sx) * 8;
-            const uint64_t* tym = tmask + (int64_t)(b - sy) * 8;
-            const uint64_t* typ = tmask + (int64_t)(b + sy) * 8;
-            uint64_t out[8];
-#pragma unroll
-            for (int lz = 0; lz < 8; ++lz) {
-                const uint64_t w = own[lz];
-                uint64_t n = w | ((w << 1) & ~COL0) | ((w >> 1) & ~COL7) | (w << 8) | (w >> 8);
-                n |= lz > 0 ? own[lz - 1] : below;
-                n |= lz < 7 ? own[lz + 1] : above;
-                if (xm) n |= (txm[lz] >> 7) & COL0;   // their lx=7 -> our lx=0
-                if (xp) n |= (txp[lz] & COL0) << 7;   // their lx=0 -> our lx=7
-                if (ym) n |= tym[lz] >> 56;           // their ly=7 -> our ly=0
-                if (yp) n |= (typ[lz] & 0xffull) << 56;
-                n &= domain_word(g, bx, by, bz, lz);
-                out[lz] = n;
-                any = any || n != 0;
-                ptsN += __popcll(n);
-                ptsT += __popcll(w);
-            }
+        }
+        return c;
+    }
+    if (wid < (int64_t)nprev * 7 + nstale) {
+        const int c = a.staleList[(int)(wid - (int64_t)nprev * 7)].quad;
+        const int cx = c % g.NQx, cy = (c / g.NQx) % g.NBy, cz = c / szq;
+        bool reached = a.prevN[c] != 0;
+        reached = reached || (cx > 0 && a.prevN[c - sxq]) || (cx < g.NQx - 1 && a.prevN[c + sxq]);
+        reached = reached || (cy > 0 && a.prevN[c - syq]) || (cy < g.NBy - 1 && a.prevN[c + syq]);
+        reached = reached || (cz > 0 && a.prevN[c - szq]) || (cz < g.NBz - 1 && a.prevN[c + szq]);
+        return reached ? -1 : c;
+    }
+    return -1;
+}
+
+// eq. 11 (R6): N = T or any in-domain face neighbour in T.  Persistent warps, one candidate quad per warp and turn.
+template <bool INCREMENTAL>
+__global__ void __launch_bounds__(kDilateWarps * 32) k_dilate_items(Geom g, DilateArgs a) {
+    __shared__ __align__(16) uint64_t s_words[kDilateWarps][32];
+    __shared__ __align__(16) uint16_t s_items[kDilateWarps][kItemsPerQuad];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int sxq = 1, syq = g.NQx, szq = g.NQx * g.NBy;
+    const int nprev = INCREMENTAL ? *a.prevCount : 0, nstale = INCREMENTAL ? *a.staleCount : 0;
+    const int64_t ncand = INCREMENTAL ? (int64_t)nprev * 7 + nstale : (int64_t)g.nquads;
+    const int64_t nwarps = (int64_t)gridDim.x * kDilateWarps;
+    auto tvalid = [&](int q) -> bool { return a.qflagT[q] != 0 && (a.tgate == nullptr || a.tgate[q] != 0); };
+    // A warp turn takes 32 consecutive candidates: each lane resolves one (which quad, does another candidate own
+    // it, can it hold an N point at all) with its flag loads in flight together; the quads that need work are
+    // then processed one after the other by the whole warp.
+    for (int64_t w0 = ((int64_t)blockIdx.x * kDilateWarps + wib) * 32; w0 < ncand; w0 += nwarps * 32) {
+    int mine = -1;
+    {
+        const int64_t wid = w0 + lane;
+        int c = -1;
+        if (wid < ncand) c = INCREMENTAL ? candidate_quad(g, a, wid, nprev, nstale) : (int)wid;
+        if (c >= 0) {
+            const int cx = c % g.NQx, cy = (c / g.NQx) % g.NBy, cz = c / szq;
+            bool any = tvalid(c);
+            any = any || (cx > 0 && tvalid(c - sxq)) || (cx < g.NQx - 1 && tvalid(c + sxq));
+            any = any || (cy > 0 && tvalid(c - syq)) || (cy < g.NBy - 1 && tvalid(c + syq));
+            any = any || (cz > 0 && tvalid(c - szq)) || (cz < g.NBz - 1 && tvalid(c + szq));
             if (any) {
+                mine = c;
+            } else {
+                // no T point in reach: the quad is outside N.  Its masks are already zero unless it was in the
+                // previous band (or, when rebuilding incrementally, in the stale band of this buffer).
+                if (INCREMENTAL || a.prevN[c]) {
+                    uint4* z = reinterpret_cast<uint4*>(a.nmask + (int64_t)c * 32);
 #pragma unroll
-                for (int i = 0; i < 4; ++i)
-                    reinterpret_cast<ulonglong2*>(nmask + (int64_t)b * 8)[i] = make_ulonglong2(out[2 * i], out[2 * i + 1]);
-            }
-        }
-        flagN[b] = any ? 1 : 0;
-    }
-    ptsT = __reduce_add_sync(0xffffffffu, ptsT);
-    ptsN = __reduce_add_sync(0xffffffffu, ptsN);
-    if ((threadIdx.x & 31) == 0) {
-        if (ptsT) atomicAdd(&counts->acc_T, (unsigned long long)ptsT);
-        if (ptsN) atomicAdd(&counts->acc_N, (unsigned long long)ptsN);
-    }
-}
-
-__device__ __forceinline__ int warp_sum(int v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-
-// Flags of this thread's 16 consecutive bricks (arrays are padded to a multiple of kScanTile with 0).
-__device__ __forceinline__ void load_flags(const uint8_t* fT, const uint8_t* fN, const uint8_t* fP, int base,
-                                           uint32_t& mT, uint32_t& mN, uint32_t& mU) {
-    const uint4 a = *reinterpret_cast<const uint4*>(fT + base);
-    const uint4 b = *reinterpret_cast<const uint4*>(fN + base);
-    const uint4 c = *reinterpret_cast<const uint4*>(fP + base);
-    const uint32_t wa[4] = {a.x, a.y, a.z, a.w}, wb[4] = {b.x, b.y, b.z, b.w}, wc[4] = {c.x, c.y, c.z, c.w};
-    mT = mN = mU = 0;
-#pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        const uint32_t t = (wa[i >> 2] >> ((i & 3) * 8)) & 0xffu;
-        const uint32_t n = (wb[i >> 2] >> ((i & 3) * 8)) & 0xffu;
-        const uint32_t p = (wc[i >> 2] >> ((i & 3) * 8)) & 0xffu;
-        mT |= (t ? 1u : 0u) << i;
-        mN |= (n ? 1u : 0u) << i;
-        mU |= ((n | p) ? 1u : 0u) << i;
-    }
-}
-
-__global__ void __launch_bounds__(kScanThreads) k_count(const uint8_t* __restrict__ fT, const uint8_t* __restrict__ fN,
-                                                        const uint8_t* __restrict__ fP, int32_t* __restrict__ partials,
-                                                        int npartials) {
-    __shared__ int red[3][kScanThreads / 32];
-    uint32_t mT, mN, mU;
-    load_flags(fT, fN, fP, blockIdx.x * kScanTile + threadIdx.x * kItemsPerThread, mT, mN, mU);
-    const int cT = warp_sum(__popc(mT)), cN = warp_sum(__popc(mN)), cU = warp_sum(__popc(mU));
-    const int w = threadIdx.x >> 5;
-    if ((threadIdx.x & 31) == 0) { red[0][w] = cT; red[1][w] = cN; red[2][w] = cU; }
-    __syncthreads();
-    if (threadIdx.x < 3) {
-        int s = 0;
-        for (int i = 0; i < kScanThreads / 32; ++i) s += red[threadIdx.x][i];
-        partials[threadIdx.x * npartials + blockIdx.x] = s;
-    }
-}
-
-// Exclusive scan of the per-CTA counts of each list, in place; totals go to Counts.  One CTA.
-__global__ void __launch_bounds__(1024) k_scan_partials(int32_t* __restrict__ partials, int npartials,
-                                                         Counts* __restrict__ counts, int iters, int count_step) {
-    __shared__ int wsum[32];
-    __shared__ int carry_s;
-    for (int l = 0; l < 3; ++l) {
-        int32_t* p = partials + l * npartials;
-        if (threadIdx.x == 0) carry_s = 0;
-        __syncthreads();
-        for (int base = 0; base < npartials; base += 1024) {
-            const int i = base + threadIdx.x;
-            const int v = i < npartials ? p[i] : 0;
-            int incl = v;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int y = __shfl_up_sync(0xffffffffu, incl, o);
-                if ((threadIdx.x & 31) >= o) incl += y;
-            }
-            if ((threadIdx.x & 31) == 31) wsum[threadIdx.x >> 5] = incl;
-            __syncthreads();
-            if (threadIdx.x < 32) {
-                int s = wsum[threadIdx.x];
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int y = __shfl_up_sync(0xffffffffu, s, o);
-                    if (threadIdx.x >= o) s += y;
+                    for (int i = 0; i < 16; ++i) z[i] = make_uint4(0u, 0u, 0u, 0u);
                 }
-                wsum[threadIdx.x] = s;  // inclusive over warps
+                a.qflagN[c] = 0;
+                a.qcount[c] = 0;
             }
-            __syncthreads();
-            const int warp_off = (threadIdx.x >> 5) ? wsum[(threadIdx.x >> 5) - 1] : 0;
-            const int carry = carry_s;
-            if (i < npartials) p[i] = carry + warp_off + incl - v;
-            __syncthreads();
-            if (threadIdx.x == 0) carry_s = carry + wsum[31];
-            __syncthreads();
         }
-        if (threadIdx.x == 0) {
-            if (l == 0) counts->nT = carry_s;
-            if (l == 1) counts->nN = carry_s;
-            if (l == 2) counts->nU = carry_s;
-        }
-        __syncthreads();
     }
-    if (threadIdx.x == 0) {   // fold the point counters of this build (k_dilate has finished: stream order)
+    unsigned todo = __ballot_sync(0xffffffffu, mine >= 0);
+    while (todo) {
+    const int src_lane = __ffs(todo) - 1;
+    todo &= todo - 1;
+    const int c = __shfl_sync(0xffffffffu, mine, src_lane);
+    __syncwarp();   // the staging of the previous quad has been copied out
+    const int qx = c % g.NQx, by = (c / g.NQx) % g.NBy, bz = c / szq;
+    const bool vs = tvalid(c);
+    const bool vxm = qx > 0 && tvalid(c - sxq), vxp = qx < g.NQx - 1 && tvalid(c + sxq);
+    const bool vym = by > 0 && tvalid(c - syq), vyp = by < g.NBy - 1 && tvalid(c + syq);
+    const bool vzm = bz > 0 && tvalid(c - szq), vzp = bz < g.NBz - 1 && tvalid(c + szq);
+    const int j = lane >> 3, lz = lane & 7;   // brick of the quad, word of the brick
+    const uint64_t w = vs ? a.tmask[(int64_t)c * 32 + lane] : 0ull;
+    uint64_t n = w | ((w << 1) & ~COL0) | ((w >> 1) & ~COL7) | (w << 8) | (w >> 8);
+    // z neighbours: the lane below / above, or the facing word of the quad below / above
+    {
+        uint64_t dn = __shfl_up_sync(0xffffffffu, w, 1), up = __shfl_down_sync(0xffffffffu, w, 1);
+        if (lz == 0) dn = vzm ? a.tmask[(int64_t)(c - szq) * 32 + j * 8 + 7] : 0ull;
+        if (lz == 7) up = vzp ? a.tmask[(int64_t)(c + szq) * 32 + j * 8 + 0] : 0ull;
+        n |= dn | up;
+    }
+    // x neighbours: brick j-1 / j+1 of this quad (8 lanes away), or brick 3 / 0 of the quad to the left / right
+    {
+        uint64_t lf = __shfl_up_sync(0xffffffffu, w, 8), rt = __shfl_down_sync(0xffffffffu, w, 8);
+        if (j == 0) lf = vxm ? a.tmask[(int64_t)(c - sxq) * 32 + 24 + lz] : 0ull;
+        if (j == 3) rt = vxp ? a.tmask[(int64_t)(c + sxq) * 32 + lz] : 0ull;
+        n |= (lf >> 7) & COL0;     // their lx = 7 -> our lx = 0
+        n |= (rt & COL0) << 7;     // their lx = 0 -> our lx = 7
+    }
+    if (vym) n |= a.tmask[(int64_t)(c - syq) * 32 + lane] >> 56;              // their ly = 7 -> our ly = 0
+    if (vyp) n |= (a.tmask[(int64_t)(c + syq) * 32 + lane] & 0xffull) << 56;  // their ly = 0 -> our ly = 7
+    n &= domain_word(g, qx * 4 + j, by, bz, lz);
+    a.nmask[(int64_t)c * 32 + lane] = n;
+    // |T|, |N|
+    {
+        const unsigned pT = __reduce_add_sync(0xffffffffu, (unsigned)__popcll(w));
+        const unsigned pN = __reduce_add_sync(0xffffffffu, (unsigned)__popcll(n));
+        if (lane == 0) {
+            if (pT) atomicAdd(&a.counts->acc_T, (unsigned long long)pT);
+            if (pN) atomicAdd(&a.counts->acc_N, (unsigned long long)pN);
+        }
+    }
+    // Item list in row-major order (lz, ly, xq): lane l takes rows (lz = l >> 2, ly = 2*(l & 3) + {0, 1}); a row's
+    // 32 bits are byte ly of word lz of the four bricks.
+    s_words[wib][lane] = n;
+    __syncwarp();
+    const unsigned char* sb = reinterpret_cast<const unsigned char*>(s_words[wib]);
+    const int rz = lane >> 2, ry = (lane & 3) * 2;
+    uint32_t row[2];
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+        const int o = rz * 8 + ry + r;
+        row[r] = (uint32_t)sb[o] | ((uint32_t)sb[64 + o] << 8) | ((uint32_t)sb[128 + o] << 16) | ((uint32_t)sb[192 + o] << 24);
+    }
+    int cnt = 0;
+#pragma unroll
+    for (int r = 0; r < 2; ++r)
+#pragma unroll
+        for (int x = 0; x < 8; ++x) cnt += ((row[r] >> (4 * x)) & 0xfu) ? 1 : 0;
+    int incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int y = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += y;
+    }
+    const int total = __shfl_sync(0xffffffffu, incl, 31);
+    int pos = incl - cnt;
+#pragma unroll
+    for (int r = 0; r < 2; ++r)
+#pragma unroll
+        for (int x = 0; x < 8; ++x) {
+            const uint32_t nib = (row[r] >> (4 * x)) & 0xfu;
+            if (nib) s_items[wib][pos++] = (uint16_t)((rz * 64 + (ry + r) * 8 + x) | (nib << 9));
+        }
+    __syncwarp();
+    // copy out in 16-byte pieces (the tail piece may carry unused entries; the slot is 1 KiB)
+    {
+        const uint4* src = reinterpret_cast<const uint4*>(s_items[wib]);
+        uint4* dst = reinterpret_cast<uint4*>(a.items + (int64_t)c * kItemsPerQuad);
+        const int pieces = (total + 7) >> 3;
+        for (int i = lane; i < pieces; i += 32) dst[i] = src[i];
+    }
+    if (lane == 0) { a.qflagN[c] = total ? 1 : 0; a.qcount[c] = total; }
+    }   // quads of this turn
+    }   // turns
+}
+
+// ---- ordered compaction of the quad flags --------------------------------------------------------
+constexpr int kCompactThreads = 1024;
+constexpr int kFlagsPerThread = 16;
+constexpr int kCompactTile = kCompactThreads * kFlagsPerThread;
+
+__device__ __forceinline__ uint32_t flag_bits16(const uint8_t* flags, int64_t base, int64_t n) {
+    uint32_t m = 0;
+    if (base + 16 <= n) {
+        const uint4 v = *reinterpret_cast<const uint4*>(flags + base);
+        const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int i = 0; i < 16; ++i) m |= (((w[i >> 2] >> ((i & 3) * 8)) & 0xffu) ? 1u : 0u) << i;
+    } else {
+        for (int i = 0; i < 16; ++i)
+            if (base + i < n && flags[base + i]) m |= 1u << i;
+    }
+    return m;
+}
+
+// CTA-wide exclusive scan of one int per thread; returns the exclusive prefix, *total = CTA sum.
+__device__ __forceinline__ int cta_exclusive_scan(int v, int* s_warp, int* total) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int incl = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int y = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += y;
+    }
+    __syncthreads();   // s_warp may still be read from a previous call
+    if (lane == 31) s_warp[w] = incl;
+    __syncthreads();
+    if (w == 0) {
+        const int x = s_warp[lane];
+        int s = x;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, s, o);
+            if (lane >= o) s += y;
+        }
+        s_warp[lane] = s - x;          // exclusive over warps
+        if (lane == 31) s_warp[32] = s; // CTA total
+    }
+    __syncthreads();
+    *total = s_warp[32];
+    return s_warp[w] + incl - v;
+}
+
+// All CTAs of the grid are co-resident (grid <= SM count, one CTA per SM fits): phase 1 counts, a grid
+// barrier on a monotone counter, phase 2 scans and scatters.  Output order = ascending quad id.
+__global__ void __launch_bounds__(kCompactThreads) k_compact(const uint8_t* __restrict__ qflagN,
+                                                             const int32_t* __restrict__ qcount, int nquads,
+                                                             QuadEntry* __restrict__ qlist, int32_t* __restrict__ partials,
+                                                             Counts* __restrict__ counts, int which,
+                                                             unsigned long long bar_target, int iters, int count_step) {
+    __shared__ int s_warp[33];
+    const int G = gridDim.x;
+    const int64_t ntiles = ((int64_t)nquads + kCompactTile - 1) / kCompactTile;
+    const int64_t tiles_per = (ntiles + G - 1) / G;
+    const int64_t t0 = (int64_t)blockIdx.x * tiles_per, t1 = min(ntiles, t0 + tiles_per);
+    // phase 1: flags of my range
+    int mine = 0;
+    for (int64_t t = t0; t < t1; ++t)
+        mine += __popc(flag_bits16(qflagN, t * kCompactTile + (int64_t)threadIdx.x * kFlagsPerThread, nquads));
+    int total;
+    cta_exclusive_scan(mine, s_warp, &total);
+    if (threadIdx.x == 0) {
+        partials[blockIdx.x] = total;
+        __threadfence();
+        atomicAdd(&counts->bar, 1ull);
+        while (*reinterpret_cast<volatile unsigned long long*>(&counts->bar) < bar_target) {}
+        __threadfence();
+    }
+    __syncthreads();
+    // phase 2: my base = sum of the partials before me
+    int base = 0;
+    {
+        int v = 0;
+        for (int i = threadIdx.x; i < (int)blockIdx.x; i += kCompactThreads) v += __ldcg(partials + i);
+        int dummy;
+        cta_exclusive_scan(v, s_warp, &dummy);
+        base = dummy;
+    }
+    if (blockIdx.x == G - 1 && threadIdx.x == 0) {
+        counts->nQ[which] = base + total;
+        // fold the point counters of this build (k_dilate_items has finished: stream order)
         counts->nT_pts = counts->acc_T;
         counts->nN_pts = counts->acc_N;
         counts->acc_T = 0;
@@ -261,93 +371,192 @@ __global__ void __launch_bounds__(1024) k_scan_partials(int32_t* __restrict__ pa
             counts->updates += counts->nT_pts + (unsigned long long)iters * counts->nN_pts;
             counts->steps += 1;
         }
+        for (int i = 0; i < kTickets; ++i) counts->ticket[i] = 0;
     }
-}
-
-// Ordered scatter of the brick ids (and packed positions) of the three lists.
-__global__ void __launch_bounds__(kScanThreads) k_scatter(const uint8_t* __restrict__ fT, const uint8_t* __restrict__ fN,
-                                                          const uint8_t* __restrict__ fP,
-                                                          const int32_t* __restrict__ partials, int npartials,
-                                                          BandBuffers bb, Geom g) {
-    __shared__ int wtot[3][kScanThreads / 32];
-    const int base = blockIdx.x * kScanTile + threadIdx.x * kItemsPerThread;
-    uint32_t m[3];
-    load_flags(fT, fN, fP, base, m[0], m[1], m[2]);
-    int excl[3];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-#pragma unroll
-    for (int l = 0; l < 3; ++l) {
-        const int c = __popc(m[l]);
-        int incl = c;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int y = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += y;
+    for (int64_t t = t0; t < t1; ++t) {
+        const int64_t first = t * kCompactTile + (int64_t)threadIdx.x * kFlagsPerThread;
+        const uint32_t m = flag_bits16(qflagN, first, nquads);
+        int tile_total;
+        int pos = base + cta_exclusive_scan(__popc(m), s_warp, &tile_total);
+        uint32_t mm = m;
+        while (mm) {
+            const int i = __ffs(mm) - 1;
+            mm &= mm - 1;
+            QuadEntry e;
+            e.quad = (int)(first + i);
+            e.nitems = qcount[first + i];
+            qlist[pos++] = e;
         }
-        if (lane == 31) wtot[l][w] = incl;
-        excl[l] = incl - c;
-    }
-    __syncthreads();
-    if ((m[0] | m[1] | m[2]) == 0) return;   // no barrier or warp collective below
-#pragma unroll
-    for (int l = 0; l < 3; ++l) {
-        int off = partials[l * npartials + blockIdx.x];
-        for (int i = 0; i < w; ++i) off += wtot[l][i];
-        excl[l] += off;
-    }
-    int bx = base % g.NBx, by = (base / g.NBx) % g.NBy, bz = base / (g.NBx * g.NBy);
-    for (int i = 0; i < kItemsPerThread; ++i) {
-        const int b = base + i;
-        const int pos = bx | (by << g.pos_sy) | (bz << g.pos_sz);
-        if (++bx == g.NBx) { bx = 0; if (++by == g.NBy) { by = 0; ++bz; } }
-        if ((m[0] >> i) & 1u) { bb.T_ids[excl[0]] = b; bb.T_pos[excl[0]++] = pos; }
-        if ((m[1] >> i) & 1u) { bb.N_ids[excl[1]] = b; bb.N_pos[excl[1]++] = pos; }
-        if ((m[2] >> i) & 1u) { bb.U_ids[excl[2]] = b; bb.U_pos[excl[2]++] = pos; }
+        base += tile_total;
     }
 }
 
-// List-ordered copies of the dense masks (ls_band_export only): one thread per (list entry, word).
-__global__ void __launch_bounds__(256) k_gather_masks(const int32_t* __restrict__ ids, const int32_t* __restrict__ count_ptr,
-                                                      const uint64_t* __restrict__ dense, uint64_t* __restrict__ out) {
-    const int64_t n = (int64_t)*count_ptr * 8;
-    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (int64_t)gridDim.x * blockDim.x)
-        out[t] = dense[(int64_t)ids[t >> 3] * 8 + (t & 7)];
+// ---- export: brick lists in ls.h's format --------------------------------------------------------
+struct ExportArgs {
+    const QuadEntry* qlist;
+    const int32_t* count;
+    const uint64_t* tmask;
+    const uint8_t* qflagT;
+    const uint8_t* tgate;
+    const uint64_t* nmask;
+    int32_t* ex_cnt;   // [2][nquads]: per list entry, T bricks / N bricks, then exclusive scans
+    int32_t* T_ids;
+    int32_t* N_ids;
+    uint64_t* T_masks;
+    uint64_t* N_masks;
+    Counts* counts;
+    int nquads;
+};
+
+// per list entry: which of the quad's 4 bricks hold T / N points (bit j)
+__device__ __forceinline__ void quad_brick_bits(const ExportArgs& a, int quad, unsigned& bT, unsigned& bN) {
+    bT = bN = 0;
+    const bool tv = a.qflagT[quad] != 0 && (a.tgate == nullptr || a.tgate[quad] != 0);
+    for (int j = 0; j < 4; ++j) {
+        uint64_t t = 0, n = 0;
+        for (int z = 0; z < 8; ++z) {
+            if (tv) t |= a.tmask[(int64_t)quad * 32 + j * 8 + z];
+            n |= a.nmask[(int64_t)quad * 32 + j * 8 + z];
+        }
+        bT |= (t ? 1u : 0u) << j;
+        bN |= (n ? 1u : 0u) << j;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_export_count(ExportArgs a) {
+    const int n = *a.count;
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
+        unsigned bT, bN;
+        quad_brick_bits(a, a.qlist[e].quad, bT, bN);
+        a.ex_cnt[e] = __popc(bT);
+        a.ex_cnt[a.nquads + e] = __popc(bN);
+    }
+}
+
+// exclusive scans of the two count arrays, in place; one CTA.
+__global__ void __launch_bounds__(1024) k_export_scan(ExportArgs a) {
+    __shared__ int s_warp[33];
+    const int n = *a.count;
+    for (int l = 0; l < 2; ++l) {
+        int32_t* p = a.ex_cnt + (int64_t)l * a.nquads;
+        int carry = 0;
+        for (int base = 0; base < n; base += 1024) {
+            const int i = base + threadIdx.x;
+            const int v = i < n ? p[i] : 0;
+            int total;
+            const int ex = cta_exclusive_scan(v, s_warp, &total);
+            if (i < n) p[i] = carry + ex;
+            carry += total;
+        }
+        if (threadIdx.x == 0) {
+            if (l == 0) a.counts->nT_bricks = carry;
+            else a.counts->nN_bricks = carry;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256) k_export_scatter(ExportArgs a, Geom g, int with_masks) {
+    const int n = *a.count;
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
+        const int quad = a.qlist[e].quad;
+        unsigned bT, bN;
+        quad_brick_bits(a, quad, bT, bN);
+        const int qx = quad % g.NQx, rest = quad / g.NQx;   // rest = bz*NBy + by
+        int pT = a.ex_cnt[e], pN = a.ex_cnt[a.nquads + e];
+        for (int j = 0; j < 4; ++j) {
+            const int b = rest * g.NBx + qx * 4 + j;   // true brick id (ls.h)
+            if ((bT >> j) & 1u) {
+                a.T_ids[pT] = b;
+                if (with_masks)
+                    for (int z = 0; z < 8; ++z) a.T_masks[(int64_t)pT * 8 + z] = a.tmask[(int64_t)quad * 32 + j * 8 + z];
+                ++pT;
+            }
+            if ((bN >> j) & 1u) {
+                a.N_ids[pN] = b;
+                if (with_masks)
+                    for (int z = 0; z < 8; ++z) a.N_masks[(int64_t)pN * 8 + z] = a.nmask[(int64_t)quad * 32 + j * 8 + z];
+                ++pN;
+            }
+        }
+    }
 }
 
 }  // namespace
 
 template <typename T>
-void launch_classify(const T* phi, const Geom& g, T gamma, const BandBuffers& bb, cudaStream_t s, int64_t* launches) {
-    const int ntx = (g.NBx + 3) / 4;
-    const int64_t ntiles = (int64_t)ntx * g.NBy * g.NBz;
+void launch_classify(const T* phi, const Geom& g, T gamma, BandBuffers& bb, cudaStream_t s, int64_t* launches) {
     const bool vec = (g.nx % 4 == 0) && ((reinterpret_cast<uintptr_t>(phi) & 15) == 0);
     if (vec)
-        k_classify<T, true><<<(unsigned)ntiles, 256, 0, s>>>(phi, g, ntx, gamma, bb.tmask, bb.flagT);
+        k_classify<T, true><<<(unsigned)g.nquads, 256, 0, s>>>(phi, g, gamma, bb.tmask[bb.tb], bb.qflagT[bb.tb]);
     else
-        k_classify<T, false><<<(unsigned)ntiles, 256, 0, s>>>(phi, g, ntx, gamma, bb.tmask, bb.flagT);
+        k_classify<T, false><<<(unsigned)g.nquads, 256, 0, s>>>(phi, g, gamma, bb.tmask[bb.tb], bb.qflagT[bb.tb]);
+    bb.tvalid_all = true;
     if (launches) *launches += 1;
 }
 
-void launch_dilate_compact(const Geom& g, const BandBuffers& bb, int iters, bool count_step, cudaStream_t s,
-                           int64_t* launches) {
-    k_dilate<<<(unsigned)((g.nbricks + 255) / 256), 256, 0, s>>>(g, bb.tmask, bb.flagT, bb.nmask, bb.flagN, bb.counts);
-    k_count<<<bb.npartials, kScanThreads, 0, s>>>(bb.flagT, bb.flagN, bb.flagNprev, bb.partials, bb.npartials);
-    k_scan_partials<<<1, 1024, 0, s>>>(bb.partials, bb.npartials, bb.counts, iters, count_step ? 1 : 0);
-    k_scatter<<<bb.npartials, kScanThreads, 0, s>>>(bb.flagT, bb.flagN, bb.flagNprev, bb.partials, bb.npartials, bb, g);
-    // Snapshot of the T masks in list order: the last reinit sweep of an incremental step overwrites the
-    // dense T masks with those of phi^{n+1}, while ls_band_export reports the band of phi^n.
-    k_gather_masks<<<sm_count() * 2, 256, 0, s>>>(bb.T_ids, &bb.counts->nT, bb.tmask, bb.T_masks);
-    if (launches) *launches += 5;
+void launch_build_lists(const Geom& g, BandBuffers& bb, bool incremental, int iters, bool count_step, cudaStream_t s,
+                        int64_t* launches) {
+    const int pv = bb.lb, cr = bb.lb ^ 1;
+    DilateArgs a;
+    a.tmask = bb.tmask[bb.tb];
+    a.qflagT = bb.qflagT[bb.tb];
+    a.tgate = bb.tvalid_all ? nullptr : bb.qflagN[pv];
+    a.prevN = bb.qflagN[pv];
+    a.prevList = bb.qlist[pv];
+    a.prevCount = &bb.counts->nQ[pv];
+    a.staleList = bb.qlist[cr];
+    a.staleCount = &bb.counts->nQ[cr];
+    a.nmask = bb.nmask;
+    a.qflagN = bb.qflagN[cr];
+    a.qcount = bb.qcount;
+    a.items = bb.items[cr];
+    a.counts = bb.counts;
+    // Persistent warps: the candidate count lives on the device (ls_step never synchronises).
+    const unsigned blocks = (unsigned)(sm_count() * 8);
+    if (incremental)
+        k_dilate_items<true><<<blocks, kDilateWarps * 32, 0, s>>>(g, a);
+    else
+        k_dilate_items<false><<<blocks, kDilateWarps * 32, 0, s>>>(g, a);
+    bb.bar_epoch += 1;
+    k_compact<<<bb.compact_grid, kCompactThreads, 0, s>>>(bb.qflagN[cr], bb.qcount, g.nquads, bb.qlist[cr], bb.partials,
+                                                          bb.counts, cr, bb.bar_epoch * (unsigned long long)bb.compact_grid,
+                                                          iters, count_step ? 1 : 0);
+    bb.lb = cr;
+    if (launches) *launches += 2;
 }
 
-void launch_gather_masks(const BandBuffers& bb, cudaStream_t s, int64_t* launches) {
-    k_gather_masks<<<sm_count() * 4, 256, 0, s>>>(bb.N_ids, &bb.counts->nN, bb.nmask, bb.N_masks);
-    if (launches) *launches += 1;
+bool launch_export(const Geom& g, BandBuffers& bb, bool with_masks, cudaStream_t s, int64_t* launches) {
+    if (!bb.ex_cnt) {
+        cudaError_t e = cudaMalloc((void**)&bb.ex_cnt, (size_t)g.nquads * 2 * sizeof(int32_t));
+        if (e == cudaSuccess) e = cudaMalloc((void**)&bb.T_ids, (size_t)g.nquads * 4 * sizeof(int32_t));
+        if (e == cudaSuccess) e = cudaMalloc((void**)&bb.N_ids, (size_t)g.nquads * 4 * sizeof(int32_t));
+        if (e == cudaSuccess) e = cudaMalloc((void**)&bb.T_masks, (size_t)g.nquads * 32 * sizeof(uint64_t));
+        if (e == cudaSuccess) e = cudaMalloc((void**)&bb.N_masks, (size_t)g.nquads * 32 * sizeof(uint64_t));
+        if (e != cudaSuccess) { cudaGetLastError(); return false; }
+    }
+    ExportArgs a;
+    a.qlist = bb.qlist[bb.lb];
+    a.count = &bb.counts->nQ[bb.lb];
+    a.tmask = bb.tmask[bb.tb];
+    a.qflagT = bb.qflagT[bb.tb];
+    a.tgate = bb.tvalid_all ? nullptr : bb.qflagN[bb.lb ^ 1];
+    a.nmask = bb.nmask;
+    a.ex_cnt = bb.ex_cnt;
+    a.T_ids = bb.T_ids;
+    a.N_ids = bb.N_ids;
+    a.T_masks = bb.T_masks;
+    a.N_masks = bb.N_masks;
+    a.counts = bb.counts;
+    a.nquads = g.nquads;
+    const int grid = sm_count() * 4;
+    k_export_count<<<grid, 256, 0, s>>>(a);
+    k_export_scan<<<1, 1024, 0, s>>>(a);
+    k_export_scatter<<<grid, 256, 0, s>>>(a, g, with_masks ? 1 : 0);
+    if (launches) *launches += 3;
+    return true;
 }
 
-int scan_tile() { return kScanTile; }
-
-template void launch_classify<float>(const float*, const Geom&, float, const BandBuffers&, cudaStream_t, int64_t*);
-template void launch_classify<double>(const double*, const Geom&, double, const BandBuffers&, cudaStream_t, int64_t*);
+template void launch_classify<float>(const float*, const Geom&, float, BandBuffers&, cudaStream_t, int64_t*);
+template void launch_classify<double>(const double*, const Geom&, double, BandBuffers&, cudaStream_t, int64_t*);
 
 }  // namespace ls

@@ -1,119 +1,145 @@
 // ls_internal.h — shared declarations of the CUDA path (libls.so).  Not part of the public ABI.
 // Nothing here is shared with oracle/ (the CPU oracle is an independent restatement of the paper).
+//
+// Band representation.  The grid is cut into 8^3 bricks (R20) and bricks into
+// QUADS: four x-adjacent bricks, 32 x 8 x 8 points, whose rows are whole 128-byte lines of an fp32
+// field.  A quad is the tile of the band kernels.  Per quad the ctx keeps
+//   * 32 T mask words and 32 N mask words (brick j = 0..3, word lz = 0..7, bit ly*8 + lx), dense by
+//     padded brick id  pb = 4*quad + j  (so a quad's masks are 256 contiguous bytes),
+//   * an ITEM LIST of the band N: one uint16 per aligned group of four x-consecutive cells that holds
+//     at least one N point (code = lz*64 + ly*8 + xq, xq = 0..7 the group within the 32-cell row;
+//     bits 9..12 = which of the four cells are in N).  One lane of a band kernel evaluates one item
+//     (two packed fp32 pairs), so lanes are 92 % full although a brick is only 56 % N points.
+// Lists of quads (ascending quad id; built by an ordered scan, no atomics-order dependence) drive the
+// band kernels; brick lists in the paper's / ls.h's format are derived on demand for ls_band_export.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 namespace ls {
 
-// Grid geometry (x fastest) and its 8^3 brick decomposition (R20).
+// Grid geometry (x fastest), its 8^3 bricks (R20) and quads of bricks.
 struct Geom {
     int nx, ny, nz;
-    int NBx, NBy, NBz;
-    int nbricks;
-    // packed brick position of the list entries (T_pos / N_pos / U_pos): bx | by << pos_sy | bz << pos_sz
-    int pos_mx, pos_my, pos_sy, pos_sz;
+    int NBx, NBy, NBz;   // bricks per axis
+    int NQx;             // quads per x row = ceil(NBx / 4)
+    int nbricks;         // NBx*NBy*NBz (true brick ids of ls.h)
+    int nquads;          // NQx*NBy*NBz
     __host__ __device__ inline int64_t idx(int i, int j, int k) const {
         return ((int64_t)k * ny + j) * nx + i;
     }
 };
 
-// Device-resident counters, written by the band builder, read by the band kernels (grid-stride
-// loops bound by these counts, so the host never needs them inside ls_step).
-struct Counts {
-    int32_t nT;            // bricks in the T list
-    int32_t nN;            // bricks in the N list
-    int32_t nU;            // bricks in the U list (N of this step  ∪  N of the previous step)
-    int32_t pad;
-    unsigned long long nT_pts, nN_pts;  // |T|, |N|
-    unsigned long long acc_T, acc_N;    // accumulators of the build in flight (k_dilate), folded by k_scan_partials
-    unsigned long long updates;         // sum over steps of |T| + iters*|N|
-    unsigned long long steps;
+constexpr int kItemsPerQuad = 512;   // 64 rows x 8 groups of 4 cells
+constexpr int kTickets = 16;
+
+// One entry of a quad list.
+struct QuadEntry {
+    int32_t quad;    // quad id
+    int32_t nitems;  // items in its list (1..512)
 };
 
-// Everything the band builder owns, as raw device pointers.
+// Device-resident counters, written by the band builder, read by the band kernels (so the host
+// never needs them inside ls_step).
+struct Counts {
+    int32_t nQ[2];         // quads in the N quad list of each list buffer
+    unsigned long long nT_pts, nN_pts;  // |T|, |N| of the band last built
+    unsigned long long acc_T, acc_N;    // accumulators of the build in flight, folded by k_compact
+    unsigned long long updates;         // sum over steps of |T| + iters*|N|
+    unsigned long long steps;
+    unsigned long long bar;             // grid barrier of k_compact (monotone)
+    unsigned int ticket[kTickets];      // dynamic tile schedulers of the band kernels of one step
+    // export scratch (ls_band_counts / ls_band_export)
+    int32_t nT_bricks, nN_bricks;
+};
+
+// Everything the band builder owns, as raw device pointers.  [2] = double buffered by step parity.
 struct BandBuffers {
-    uint64_t* tmask;   // [nbricks*8] dense T mask words; valid only where flagT != 0
-    uint64_t* nmask;   // [nbricks*8] dense N mask words; valid only where flagN != 0
-    uint8_t* flagT;    // [nbricks]
-    uint8_t* flagN;    // [nbricks] N flags of the band being built
-    uint8_t* flagNprev;// [nbricks] N flags of the previous step's band (all 0 at the start of a call)
-    int32_t* T_ids;    // [nbricks]
-    uint64_t* T_masks; // [nbricks*8] list-ordered snapshot of the T masks (export); N_masks: filled at export
-    int32_t* N_ids;
-    uint64_t* N_masks;
-    int32_t* U_ids;
-    int32_t* T_pos;    // [nbricks] packed (bx, by, bz) of each list entry, see Geom::pos_*
-    int32_t* N_pos;
-    int32_t* U_pos;
-    int32_t* partials; // [3 * npartials] per-CTA flag counts, then their exclusive scans
-    int npartials;
+    uint64_t* tmask[2];   // [nquads*32] T mask words.  Buffer `tb` holds T of the band last built; the last
+                          // sweep of an incremental step writes T of phi^{n+1} into the other one, which the
+                          // next step adopts (tb ^= 1) before its Advance.
+    uint8_t* qflagT[2];   // [nquads] quad holds a T point (valid as tmask is, see tvalid_all)
+    uint64_t* nmask;      // [nquads*32] N mask words of the band last built; all-zero for quads outside N
+    uint8_t* qflagN[2];   // [nquads] quad holds an N point, per list buffer
+    uint16_t* items[2];   // [nquads*512] item lists, dense by quad id, per list buffer
+    int32_t* qcount;      // [nquads] items of the quad in the band being built
+    QuadEntry* qlist[2];  // [nquads] N quad list per list buffer
+    int32_t* partials;    // [<= 1024] per-CTA counts of k_compact
     Counts* counts;
+    // export scratch, allocated on first use: brick-level lists in ls.h's format
+    int32_t* ex_cnt;      // [2*nquads] per listed quad: T bricks, N bricks (then their exclusive scans)
+    int32_t* T_ids;
+    int32_t* N_ids;
+    uint64_t* T_masks;
+    uint64_t* N_masks;
+    // host-side state
+    int tb;               // T buffer of the band last built
+    int lb;               // list buffer of the band last built
+    bool tvalid_all;      // tmask[tb] / qflagT[tb] valid for every quad (after a whole-grid classify); otherwise
+                          // only for quads with qflagN[lb ^ 1] (emitted by the last sweep over that band)
+    unsigned long long bar_epoch;   // launches of k_compact so far
+    int compact_grid;
 };
 
 // ---- band builder (ls_band.cu) --------------------------------------------------------------
-// Full-grid classification |phi| < gamma into per-brick T masks (eq. 6).
+// Whole-grid classification |phi| < gamma into tmask[bb.tb] / qflagT[bb.tb] (eq. 6); sets tvalid_all.
 template <typename T>
-void launch_classify(const T* phi, const Geom& g, T gamma, const BandBuffers& bb, cudaStream_t s, int64_t* launches);
-// N = one-cell face dilation of T (eq. 11), then ordered compaction of the T, N and U lists.
+void launch_classify(const T* phi, const Geom& g, T gamma, BandBuffers& bb, cudaStream_t s, int64_t* launches);
+// N = one-cell face dilation of T (eq. 11) for every quad that can hold N points, item lists, then the
+// ordered quad list, into list buffer lb ^ 1, which becomes lb.  `incremental`: visit only the quads of the
+// previous band and their face neighbours (T^{n+1} is a subset of N^n); else every quad.
 // `iters` only feeds the update counter (|T| + iters*|N|).
-void launch_dilate_compact(const Geom& g, const BandBuffers& bb, int iters, bool count_step, cudaStream_t s,
-                           int64_t* launches);
+void launch_build_lists(const Geom& g, BandBuffers& bb, bool incremental, int iters, bool count_step, cudaStream_t s,
+                        int64_t* launches);
+// Brick lists of the band last built in ls.h's format into T_ids / T_masks / N_ids / N_masks and the brick
+// counts into Counts (allocates the export scratch on first use; returns false if that fails).
+bool launch_export(const Geom& g, BandBuffers& bb, bool with_masks, cudaStream_t s, int64_t* launches);
 
-// List-ordered copy N_masks of the dense N masks of the band last built (for ls_band_export; T_masks is
-// snapshotted by launch_dilate_compact).
-void launch_gather_masks(const BandBuffers& bb, cudaStream_t s, int64_t* launches);
-
-// ---- stencil kernels (ls_stencil.cu) --------------------------------------------------------
+// ---- stencil parameters -----------------------------------------------------------------------
 template <typename T>
 struct StencilParams {
     T inv_dx;      // 1/dx
+    T half_inv_dx; // inv_dx / 2 (exact)
     T dx2;         // dx*dx
     T dt;          // dt (advance) or dtau (reinit)
     T beta, gamma, three_beta, inv3;  // eq. 7 constants, inv3 = 1/((gamma-beta)^3)
 };
 
-// Advance over the U list: writes every in-domain point of each listed brick (T points by eq. 8,
-// the rest copied).  src = phi^n, dst = phi_bar.
+// What one launch of a band kernel does to the band (ls_tile.cu, ls_stencil.cu).
+struct BandOp {
+    bool advance = false;   // Step 2 (eq. 3/8) on the T bits of the items; other cells of an item are copied
+    int sweeps = 0;         // Step 3 sweeps (eq. 12-13) fused after it (temporal blocking); advance + sweeps >= 1
+    bool copy = false;      // neither: dst = src on the item cells (scalar path only; with clamp: eq. 10)
+    bool clamp = false;     // eq. 10 on the values written
+    bool emit_T = false;    // also emit the T masks of the values written into tmask[tb ^ 1] (requires clamp)
+    unsigned long long* residual = nullptr;   // max |d_new - d_old| over N of the LAST sweep, as ordered bits
+    int list = 0;           // list buffer to iterate (quads + items)
+    const uint8_t* tgate = nullptr;   // advance: null, or tmask[tb] is valid only for quads with tgate != 0
+    bool reverse = false;   // walk the list from its end (L2 reuse between consecutive launches)
+};
+
+// Band kernel over a quad list: reads `src` (and F), writes the item cells of `dst`.
+// Returns false if the tile path cannot address the grid (caller falls back to the scalar kernels).
 template <typename T>
-void launch_advance_band(const T* phi, const T* F, T* out, const Geom& g, const StencilParams<T>& p,
-                         const BandBuffers& bb, bool use_T_list, cudaStream_t s, int64_t* launches);
+bool launch_band_tile(const T* src, const T* F, T* dst, const Geom& g, const StencilParams<T>& p, const BandBuffers& bb,
+                      const BandOp& op, cudaStream_t s, int64_t* launches);
+template <typename T>
+bool tile_usable(const Geom& g, const void* a, const void* b, const void* c);
+// Scalar fallback (any nx, any alignment): one launch = advance OR one sweep OR a copy (even `iters`: eq. 10 only).
+template <typename T>
+void launch_band_scalar(const T* src, const T* F, T* dst, const Geom& g, const StencilParams<T>& p, const BandBuffers& bb,
+                        const BandOp& op, cudaStream_t s, int64_t* launches);
+
 // Dense full-domain advance (c == 1), cfg 2.
 template <typename T>
 void launch_advance_dense(const T* phi, const T* F, T* out, const Geom& g, const StencilParams<T>& p,
                           cudaStream_t s, int64_t* launches);
-// One reinit sweep over the N list: dst(x) = update(src)(x) for x in N; rows of a listed brick that
-// hold an N point are written whole (non-N points of such a row keep src's value).
-//   clamp        : apply eq. 10 to the values written (last sweep of a step)
-//   residual     : if non-null, atomically max-accumulates |dst - src| over N as ordered bits
-//   emit_T       : if true, also emits the T mask words / flagT of phi^{n+1} = clamp(dst) per N brick
-//                  (incremental rebuild; requires clamp)
-template <typename T>
-void launch_reinit_band(const T* src, T* dst, const Geom& g, const StencilParams<T>& p, const BandBuffers& bb,
-                        bool clamp, unsigned long long* residual, bool emit_T, cudaStream_t s, int64_t* launches);
-// dst(x) = clamp(src(x)) on the rows of N bricks that hold N points (even `iters`, iters = 0).
-template <typename T>
-void launch_copy_clamp_band(const T* src, T* dst, const Geom& g, T gamma, const BandBuffers& bb, cudaStream_t s,
-                            int64_t* launches);
 // eq. 10 at every point of a; where the value changes it is also written to b (b may be null).
 template <typename T>
 void launch_clamp_all(T* a, T* b, int64_t n, T gamma, cudaStream_t s, int64_t* launches);
 
-// ---- TMA-pipelined band kernels (ls_tma.cu) ---------------------------------------------------
-// Usable when every field row starts on a 16-byte boundary (nx*sizeof(T) % 16 == 0, aligned bases) and
-// the driver exposes cuTensorMapEncodeTiled.  The launchers return false (nothing enqueued) if the
-// tensor map cannot be built; the callers then take the scalar kernels of ls_stencil.cu.
-template <typename T>
-bool tma_usable(const Geom& g, const void* a, const void* b, const void* c);
-template <typename T>
-bool launch_reinit_tma(const T* src, T* dst, const Geom& g, const StencilParams<T>& p, const BandBuffers& bb,
-                       bool clamp, unsigned long long* residual, bool emit_T, cudaStream_t s, int64_t* launches);
-template <typename T>
-bool launch_advance_tma(const T* phi, const T* F, T* out, const Geom& g, const StencilParams<T>& p,
-                        const BandBuffers& bb, bool use_T_list, cudaStream_t s, int64_t* launches);
-
-// Bit-for-bit check of the packed pair arithmetic against the scalar functions on n random stencil pairs.
-// mismatches: 2 counters (differing results; differing samples); dbg: 26 floats of the first differing sample or null.
+// Bit-for-bit check of the packed arithmetic against the scalar functions on n random stencil samples.
+// mismatches: 2 counters (differing results; differing samples); dbg: 32 floats of the first differing sample or null.
 void launch_selftest_math(uint64_t seed, int64_t n, const StencilParams<float>& p, unsigned long long* mismatches,
                           float* dbg, cudaStream_t s);
 

@@ -39,102 +39,99 @@ __device__ __forceinline__ void load_halo_tile(T* __restrict__ s, const T* __res
 
 #define LS_TILE(s, lx, ly, lz) (s)[(((lz) + 1) * kTileEdge + ((ly) + 1)) * kTileEdge + ((lx) + 1)]
 
-// Advance over a brick list.  Writes every in-domain point of each listed brick.
-template <typename T>
-__global__ void __launch_bounds__(kBandThreads) k_advance_band(const T* __restrict__ phi, const T* __restrict__ F,
-                                                               T* __restrict__ out, Geom g, StencilParams<T> p,
-                                                               const int32_t* __restrict__ ids,
-                                                               const int32_t* __restrict__ count_ptr,
-                                                               const uint64_t* __restrict__ list_masks,
-                                                               const uint64_t* __restrict__ tmask,
-                                                               const uint8_t* __restrict__ flagT) {
-    __shared__ T s[kTileElems];
-    const int count = *count_ptr;
-    const int lx = threadIdx.x & 7, ly = (threadIdx.x >> 3) & 7, lz0 = threadIdx.x >> 6;
-    for (int li = blockIdx.x; li < count; li += gridDim.x) {
-        const int b = ids[li];
-        const int bx = b % g.NBx, by = (b / g.NBx) % g.NBy, bz = b / (g.NBx * g.NBy);
-        const int x0 = bx * 8, y0 = by * 8, z0 = bz * 8;
-        load_halo_tile(s, phi, g, x0, y0, z0);
-        const bool has_T = list_masks ? true : (flagT[b] != 0);
-        __syncthreads();
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int lz = lz0 + 4 * h;
-            const int i = x0 + lx, j = y0 + ly, k = z0 + lz;
-            if (i < g.nx && j < g.ny && k < g.nz) {
-                uint64_t w = 0;
-                if (has_T) w = (list_masks ? list_masks : tmask)[(int64_t)b * 8 + lz];   // both dense per brick
-                const T c = LS_TILE(s, lx, ly, lz);
-                T v = c;
-                const int64_t at = g.idx(i, j, k);
-                if ((w >> (ly * 8 + lx)) & 1ull) {
-                    v = advance_value<T, false>(c, LS_TILE(s, lx - 1, ly, lz), LS_TILE(s, lx + 1, ly, lz),
-                                                LS_TILE(s, lx, ly - 1, lz), LS_TILE(s, lx, ly + 1, lz),
-                                                LS_TILE(s, lx, ly, lz - 1), LS_TILE(s, lx, ly, lz + 1), __ldg(F + at), p);
-                }
-                out[at] = v;
-            }
-        }
-        __syncthreads();
-    }
-}
+enum ScalarMode { kAdvance = 0, kReinit = 1, kCopy = 2 };
 
-// One reinit sweep over the N list (see launch_reinit_band in ls_internal.h).
-template <typename T, bool CLAMP, bool RESIDUAL, bool EMIT_T>
-__global__ void __launch_bounds__(kBandThreads) k_reinit_band(const T* __restrict__ src, T* __restrict__ dst, Geom g,
-                                                              StencilParams<T> p, const int32_t* __restrict__ ids,
-                                                              const int32_t* __restrict__ count_ptr,
-                                                              const uint64_t* __restrict__ masks,
-                                                              unsigned long long* __restrict__ residual,
-                                                              uint64_t* __restrict__ tmask, uint8_t* __restrict__ flagT) {
+struct ScalarArgs {
+    const QuadEntry* qlist;
+    const int32_t* count;
+    const uint64_t* nmask;        // N masks of the band the list describes
+    const uint64_t* tmask_in;     // kAdvance: T masks
+    const uint8_t* qflagT_in;
+    const uint8_t* tgate;
+    uint64_t* tmask_out;          // EMIT_T
+    uint8_t* qflagT_out;
+    unsigned long long* residual;
+};
+
+// Scalar band kernel for grids the tile path cannot address: one CTA per listed quad and turn, one thread per
+// cell of a brick layer pair, brick by brick.  Same arithmetic (scalar functions of ls_math.cuh), same writes:
+// every N cell of the quad gets the new value (kAdvance: N cells outside T are copied).
+template <typename T, int MODE, bool CLAMP, bool RESIDUAL, bool EMIT_T>
+__global__ void __launch_bounds__(kBandThreads) k_band_scalar(const T* __restrict__ src, const T* __restrict__ F,
+                                                              T* __restrict__ dst, Geom g, StencilParams<T> p,
+                                                              ScalarArgs a) {
     __shared__ T s[kTileElems];
     __shared__ uint32_t halves[8][2];
-    const int count = *count_ptr;
+    __shared__ int s_any;
+    const int count = *a.count;
     const int lx = threadIdx.x & 7, ly = (threadIdx.x >> 3) & 7, lz0 = threadIdx.x >> 6;
     T rmax = T(0);
     for (int li = blockIdx.x; li < count; li += gridDim.x) {
-        const int b = ids[li];
-        const int bx = b % g.NBx, by = (b / g.NBx) % g.NBy, bz = b / (g.NBx * g.NBy);
-        const int x0 = bx * 8, y0 = by * 8, z0 = bz * 8;
-        load_halo_tile(s, src, g, x0, y0, z0);
-        __syncthreads();
+        const int quad = a.qlist[li].quad;
+        const int qx = quad % g.NQx, rest = quad / g.NQx, by = rest % g.NBy, bz = rest / g.NBy;
+        bool tvalid = false;
+        if (MODE == kAdvance) tvalid = a.qflagT_in[quad] != 0 && (a.tgate == nullptr || a.tgate[quad] != 0);
+        if (EMIT_T && threadIdx.x == 0) s_any = 0;
+        for (int j = 0; j < 4; ++j) {
+            const int bx = qx * 4 + j;
+            const uint64_t* nw = a.nmask + (int64_t)quad * 32 + j * 8;
+            uint64_t any = 0;
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int lz = lz0 + 4 * h;
-            const int i = x0 + lx, j = y0 + ly, k = z0 + lz;
-            const uint64_t w = masks[(int64_t)b * 8 + lz];   // dense per-brick N masks
-            const unsigned rowbits = (unsigned)(w >> (ly * 8)) & 0xffu;
-            const bool active = (rowbits >> lx) & 1u;
-            bool tbit = false;
-            if (rowbits != 0 && i < g.nx && j < g.ny && k < g.nz) {
-                const T c = LS_TILE(s, lx, ly, lz);
-                T v = c;
-                if (active) {
-                    v = reinit_value<T>(c, LS_TILE(s, lx - 1, ly, lz), LS_TILE(s, lx + 1, ly, lz),
-                                        LS_TILE(s, lx, ly - 1, lz), LS_TILE(s, lx, ly + 1, lz),
-                                        LS_TILE(s, lx, ly, lz - 1), LS_TILE(s, lx, ly, lz + 1), p);
-                    if (RESIDUAL) rmax = fmax(rmax, mag(v - c));
+            for (int z = 0; z < 8; ++z) any |= nw[z];
+            if (any == 0) {   // uniform over the CTA
+                if (EMIT_T && threadIdx.x < 8) a.tmask_out[(int64_t)quad * 32 + j * 8 + threadIdx.x] = 0ull;
+                continue;
+            }
+            const int x0 = bx * 8, y0 = by * 8, z0 = bz * 8;
+            __syncthreads();   // the tile of the previous brick has been read
+            if (MODE != kCopy) load_halo_tile(s, src, g, x0, y0, z0);
+            __syncthreads();
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int lz = lz0 + 4 * h;
+                const int i = x0 + lx, jj = y0 + ly, k = z0 + lz;
+                const bool nbit = (nw[lz] >> (ly * 8 + lx)) & 1ull;   // in-domain by construction
+                bool tbit = false;
+                if (nbit) {
+                    const int64_t at = g.idx(i, jj, k);
+                    const T c = MODE == kCopy ? src[at] : LS_TILE(s, lx, ly, lz);
+                    T v = c;
+                    if (MODE == kAdvance) {
+                        const bool t = tvalid && ((a.tmask_in[(int64_t)quad * 32 + j * 8 + lz] >> (ly * 8 + lx)) & 1ull);
+                        if (t)
+                            v = advance_value<T, false>(c, LS_TILE(s, lx - 1, ly, lz), LS_TILE(s, lx + 1, ly, lz),
+                                                        LS_TILE(s, lx, ly - 1, lz), LS_TILE(s, lx, ly + 1, lz),
+                                                        LS_TILE(s, lx, ly, lz - 1), LS_TILE(s, lx, ly, lz + 1), __ldg(F + at), p);
+                    } else if (MODE == kReinit) {
+                        v = reinit_value<T>(c, LS_TILE(s, lx - 1, ly, lz), LS_TILE(s, lx + 1, ly, lz),
+                                            LS_TILE(s, lx, ly - 1, lz), LS_TILE(s, lx, ly + 1, lz),
+                                            LS_TILE(s, lx, ly, lz - 1), LS_TILE(s, lx, ly, lz + 1), p);
+                        if (RESIDUAL) rmax = fmax(rmax, mag(v - c));
+                    }
+                    if (CLAMP) v = clamp_val(v, p.gamma);
+                    if (EMIT_T) tbit = mag(v) < p.gamma;
+                    dst[at] = v;
                 }
-                if (CLAMP) v = clamp_val(v, p.gamma);
-                if (EMIT_T) tbit = active && mag(v) < p.gamma;
-                dst[g.idx(i, j, k)] = v;
+                if (EMIT_T) {
+                    // this warp holds rows 4*(warp&1) .. +3 of layer lz: lane == bit index within the half word
+                    const unsigned hw = __ballot_sync(0xffffffffu, tbit);
+                    if ((threadIdx.x & 31) == 0) halves[lz][(threadIdx.x >> 5) & 1] = hw;
+                }
             }
             if (EMIT_T) {
-                // this warp holds rows 4*(warp&1) .. +3 of layer lz: lane == bit index within the half word
-                const unsigned hw = __ballot_sync(0xffffffffu, tbit);
-                if ((threadIdx.x & 31) == 0) halves[lz][(threadIdx.x >> 5) & 1] = hw;
+                __syncthreads();
+                if (threadIdx.x < 8) {
+                    const uint64_t word = (uint64_t)halves[threadIdx.x][0] | ((uint64_t)halves[threadIdx.x][1] << 32);
+                    a.tmask_out[(int64_t)quad * 32 + j * 8 + threadIdx.x] = word;
+                    if (word) s_any = 1;
+                }
             }
         }
-        __syncthreads();
-        if (EMIT_T && threadIdx.x < 32) {
-            uint64_t word = 0;
-            if (threadIdx.x < 8) word = (uint64_t)halves[threadIdx.x][0] | ((uint64_t)halves[threadIdx.x][1] << 32);
-            const bool any = __ballot_sync(0xffffffffu, word != 0) != 0;
-            if (threadIdx.x < 8 && any) tmask[(int64_t)b * 8 + threadIdx.x] = word;
-            if (threadIdx.x == 0) flagT[b] = any ? 1 : 0;
+        if (EMIT_T) {
+            __syncthreads();
+            if (threadIdx.x == 0) a.qflagT_out[quad] = s_any ? 1 : 0;
+            __syncthreads();
         }
-        if (EMIT_T) __syncthreads();
     }
     if (RESIDUAL) {
         // non-negative IEEE values order like their bit patterns
@@ -146,30 +143,7 @@ __global__ void __launch_bounds__(kBandThreads) k_reinit_band(const T* __restric
             const unsigned long long y = __shfl_xor_sync(0xffffffffu, bits, o);
             bits = y > bits ? y : bits;
         }
-        if ((threadIdx.x & 31) == 0 && bits != 0) atomicMax(residual, bits);
-    }
-}
-
-template <typename T>
-__global__ void __launch_bounds__(kBandThreads) k_copy_clamp_band(const T* __restrict__ src, T* __restrict__ dst, Geom g,
-                                                                  T gamma, const int32_t* __restrict__ ids,
-                                                                  const int32_t* __restrict__ count_ptr,
-                                                                  const uint64_t* __restrict__ masks) {
-    const int count = *count_ptr;
-    const int lx = threadIdx.x & 7, ly = (threadIdx.x >> 3) & 7, lz0 = threadIdx.x >> 6;
-    for (int li = blockIdx.x; li < count; li += gridDim.x) {
-        const int b = ids[li];
-        const int bx = b % g.NBx, by = (b / g.NBx) % g.NBy, bz = b / (g.NBx * g.NBy);
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int lz = lz0 + 4 * h;
-            const int i = bx * 8 + lx, j = by * 8 + ly, k = bz * 8 + lz;
-            const uint64_t w = masks[(int64_t)b * 8 + lz];   // dense per-brick N masks
-            if (((w >> (ly * 8)) & 0xffull) != 0 && i < g.nx && j < g.ny && k < g.nz) {
-                const int64_t at = g.idx(i, j, k);
-                dst[at] = clamp_val(src[at], gamma);
-            }
-        }
+        if ((threadIdx.x & 31) == 0 && bits != 0) atomicMax(a.residual, bits);
     }
 }
 
@@ -319,38 +293,49 @@ __global__ void __launch_bounds__(256) k_selftest_math(uint64_t seed, int64_t n,
             const uint64_t rf = mix64(r + 9);
             f[h] = (rf & 15) == 0 ? 0.f : ((float)(rf >> 40) * (1.0f / 8388608.0f) - 1.0f);
         }
-        const float* a = line;
-        const float* b = line + 8;
-        const float r0 = reinit_value<float>(a[3], a[2], a[4], a[1], a[5], a[0], a[6], p);
-        const float r1 = reinit_value<float>(b[3], b[2], b[4], b[1], b[5], b[0], b[6], p);
-        const float a0 = advance_value<float, false>(a[3], a[2], a[4], a[1], a[5], a[0], a[6], f[0], p);
-        const float a1 = advance_value<float, false>(b[3], b[2], b[4], b[1], b[5], b[0], b[6], f[1], p);
-        const Two<float> rp = reinit_pair<float>(line, 3, 11, 2, 3, p);
-        const Two<float> ap = advance_pair<float>(line, 3, 11, 2, 3, f[0], f[1], p);
-        const float e0 = advance_value<float, true>(a[3], a[2], a[4], a[1], a[5], a[0], a[6], f[0], p);
-        const float e1 = advance_value<float, true>(b[3], b[2], b[4], b[1], b[5], b[0], b[6], f[1], p);
-        const float2 dp = advance_dense_pair(make_float2(a[3], b[3]), make_float2(a[2], b[2]), make_float2(a[4], b[4]),
-                                             make_float2(a[1], b[1]), make_float2(a[5], b[5]), make_float2(a[0], b[0]),
-                                             make_float2(a[6], b[6]), make_float2(f[0], f[1]), p);
-        const int br = !same_bits(rp.x, r0) + !same_bits(rp.y, r1),
-                  ba = !same_bits(ap.x, a0) + !same_bits(ap.y, a1) + !same_bits(dp.x, e0) + !same_bits(dp.y, e1);
+        // The item under test: cells 0,1 = the two random stencils, cells 2,3 = the same two swapped, so both
+        // packed pairs and both halves see every sample; x neighbours of an item are its own cells, which the
+        // scalar reference below reads the same way.
+        const float* A = line;
+        const float* B = line + 8;
+        Item4<float> it;
+        const float* src[4] = {A, B, B, A};
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            it.c[e] = src[e][3]; it.ym[e] = src[e][1]; it.yp[e] = src[e][5]; it.zm[e] = src[e][0]; it.zp[e] = src[e][6];
+        }
+        it.xm = A[2];
+        it.xp = A[4];
+        const float ff[4] = {f[0], f[1], f[1], f[0]};
+        float rr[4], ra[4], rd[4], pr_[4], pa_[4], pd_[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const float l = it.left(e), r = it.right(e);
+            rr[e] = reinit_value<float>(it.c[e], l, r, it.ym[e], it.yp[e], it.zm[e], it.zp[e], p);
+            ra[e] = advance_value<float, false>(it.c[e], l, r, it.ym[e], it.yp[e], it.zm[e], it.zp[e], ff[e], p);
+            rd[e] = advance_value<float, true>(it.c[e], l, r, it.ym[e], it.yp[e], it.zm[e], it.zp[e], ff[e], p);
+        }
+        reinit_item<float>(it, p, pr_);
+        advance_item<float, false>(it, ff, p, pa_);
+        advance_item<float, true>(it, ff, p, pd_);
+        int br = 0, ba = 0;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            br += !same_bits(pr_[e], rr[e]);
+            ba += !same_bits(pa_[e], ra[e]) + !same_bits(pd_[e], rd[e]);
+        }
         bad += br + ba;
         if (dbg && (br | ba) && atomicAdd(mismatches + 1, 1ull) == 0) {   // first failing sample, for debugging
             for (int k = 0; k < 16; ++k) dbg[k] = line[k];
-            dbg[16] = f[0]; dbg[17] = f[1]; dbg[18] = r0; dbg[19] = r1; dbg[20] = rp.x; dbg[21] = rp.y;
-            dbg[22] = a0; dbg[23] = a1; dbg[24] = ap.x; dbg[25] = ap.y;
+            dbg[16] = f[0]; dbg[17] = f[1];
+            for (int e = 0; e < 4; ++e) { dbg[18 + e] = rr[e]; dbg[22 + e] = pr_[e]; }
+            dbg[26] = ra[0]; dbg[27] = pa_[0]; dbg[28] = ra[1]; dbg[29] = pa_[1]; dbg[30] = rd[0]; dbg[31] = pd_[0];
         }
     }
     if (bad) atomicAdd(mismatches, bad);
 }
 
 int band_grid() { return sm_count() * 8; }
-
-// Debug knob: LS_DISABLE_TMA=1 forces the scalar kernels (A/B timing, parity of the two paths).
-bool tma_disabled() {
-    static const bool off = [] { const char* e = getenv("LS_DISABLE_TMA"); return e && e[0] == '1'; }();
-    return off;
-}
 
 }  // namespace
 
@@ -371,17 +356,31 @@ int sm_count() {
 }
 
 template <typename T>
-void launch_advance_band(const T* phi, const T* F, T* out, const Geom& g, const StencilParams<T>& p,
-                         const BandBuffers& bb, bool use_T_list, cudaStream_t s, int64_t* launches) {
-    if (!tma_disabled() && tma_usable<T>(g, phi, F, out) &&
-        launch_advance_tma<T>(phi, F, out, g, p, bb, use_T_list, s, launches))
-        return;
-    if (use_T_list)
-        k_advance_band<T><<<band_grid(), kBandThreads, 0, s>>>(phi, F, out, g, p, bb.T_ids, &bb.counts->nT, bb.tmask,
-                                                               nullptr, nullptr);
-    else
-        k_advance_band<T><<<band_grid(), kBandThreads, 0, s>>>(phi, F, out, g, p, bb.U_ids, &bb.counts->nU, nullptr,
-                                                               bb.tmask, bb.flagT);
+void launch_band_scalar(const T* src, const T* F, T* dst, const Geom& g, const StencilParams<T>& p, const BandBuffers& bb,
+                        const BandOp& op, cudaStream_t s, int64_t* launches) {
+    ScalarArgs a;
+    a.qlist = bb.qlist[op.list];
+    a.count = &bb.counts->nQ[op.list];
+    a.nmask = bb.nmask;
+    a.tmask_in = bb.tmask[bb.tb];
+    a.qflagT_in = bb.qflagT[bb.tb];
+    a.tgate = op.tgate;
+    a.tmask_out = bb.tmask[bb.tb ^ 1];
+    a.qflagT_out = bb.qflagT[bb.tb ^ 1];
+    a.residual = op.residual;
+    const int grid = band_grid();
+#define LS_LAUNCH(M, C, R, E) k_band_scalar<T, M, C, R, E><<<grid, kBandThreads, 0, s>>>(src, F, dst, g, p, a)
+    if (op.advance) LS_LAUNCH(kAdvance, false, false, false);
+    else if (op.copy) {
+        if (op.emit_T) LS_LAUNCH(kCopy, true, false, true);
+        else if (op.clamp) LS_LAUNCH(kCopy, true, false, false);
+        else LS_LAUNCH(kCopy, false, false, false);
+    } else if (op.emit_T) LS_LAUNCH(kReinit, true, false, true);
+    else if (op.residual && op.clamp) LS_LAUNCH(kReinit, true, true, false);
+    else if (op.residual) LS_LAUNCH(kReinit, false, true, false);
+    else if (op.clamp) LS_LAUNCH(kReinit, true, false, false);
+    else LS_LAUNCH(kReinit, false, false, false);
+#undef LS_LAUNCH
     if (launches) *launches += 1;
 }
 
@@ -404,33 +403,6 @@ void launch_advance_dense(const T* phi, const T* F, T* out, const Geom& g, const
 }
 
 template <typename T>
-void launch_reinit_band(const T* src, T* dst, const Geom& g, const StencilParams<T>& p, const BandBuffers& bb,
-                        bool clamp, unsigned long long* residual, bool emit_T, cudaStream_t s, int64_t* launches) {
-    if (!tma_disabled() && tma_usable<T>(g, src, dst, nullptr) &&
-        launch_reinit_tma<T>(src, dst, g, p, bb, clamp, residual, emit_T, s, launches))
-        return;
-    const int grid = band_grid();
-    const int32_t* cnt = &bb.counts->nN;
-#define LS_LAUNCH(C, R, E)                                                                                        \
-    k_reinit_band<T, C, R, E><<<grid, kBandThreads, 0, s>>>(src, dst, g, p, bb.N_ids, cnt, bb.nmask, residual,   \
-                                                            bb.tmask, bb.flagT)
-    if (emit_T) LS_LAUNCH(true, false, true);
-    else if (residual && clamp) LS_LAUNCH(true, true, false);
-    else if (residual) LS_LAUNCH(false, true, false);
-    else if (clamp) LS_LAUNCH(true, false, false);
-    else LS_LAUNCH(false, false, false);
-#undef LS_LAUNCH
-    if (launches) *launches += 1;
-}
-
-template <typename T>
-void launch_copy_clamp_band(const T* src, T* dst, const Geom& g, T gamma, const BandBuffers& bb, cudaStream_t s,
-                            int64_t* launches) {
-    k_copy_clamp_band<T><<<band_grid(), kBandThreads, 0, s>>>(src, dst, g, gamma, bb.N_ids, &bb.counts->nN, bb.nmask);
-    if (launches) *launches += 1;
-}
-
-template <typename T>
 void launch_clamp_all(T* a, T* b, int64_t n, T gamma, cudaStream_t s, int64_t* launches) {
     const int grid = sm_count() * 16;
     if (sizeof(T) == 4 && n % 4 == 0 && (reinterpret_cast<uintptr_t>(a) & 15) == 0 &&
@@ -444,14 +416,10 @@ void launch_clamp_all(T* a, T* b, int64_t n, T gamma, cudaStream_t s, int64_t* l
 }
 
 #define LS_INSTANTIATE(T)                                                                                          \
-    template void launch_advance_band<T>(const T*, const T*, T*, const Geom&, const StencilParams<T>&,            \
-                                         const BandBuffers&, bool, cudaStream_t, int64_t*);                        \
+    template void launch_band_scalar<T>(const T*, const T*, T*, const Geom&, const StencilParams<T>&,             \
+                                        const BandBuffers&, const BandOp&, cudaStream_t, int64_t*);                \
     template void launch_advance_dense<T>(const T*, const T*, T*, const Geom&, const StencilParams<T>&,           \
                                           cudaStream_t, int64_t*);                                                 \
-    template void launch_reinit_band<T>(const T*, T*, const Geom&, const StencilParams<T>&, const BandBuffers&,   \
-                                        bool, unsigned long long*, bool, cudaStream_t, int64_t*);                  \
-    template void launch_copy_clamp_band<T>(const T*, T*, const Geom&, T, const BandBuffers&, cudaStream_t,       \
-                                            int64_t*);                                                             \
     template void launch_clamp_all<T>(T*, T*, int64_t, T, cudaStream_t, int64_t*);
 LS_INSTANTIATE(float)
 LS_INSTANTIATE(double)

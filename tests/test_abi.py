@@ -83,12 +83,15 @@ def test_product_does_not_import_oracle():
 
 
 def test_packed_fp32_arithmetic_is_not_contracted():
-    """The fp32 band kernels use packed FMUL2 / FADD2 / FFMA2.  ptxas 12.9 contracts mul.rn.f32x2 +
-    add.rn.f32x2 into FFMA2 even under -fmad=false, which would break the arithmetic contract (R18: no
-    FMA contraction); ls_math.cuh routes every sum of a product through scalar adds to prevent it.
-    The only FFMA2 left are the explicit ones of the correctly rounded sqrt (2 per pair) and divide (5 per
-    pair) sequences: 2 evaluation rounds x (2 sqrt + 1 div) = 18 in a reinit kernel, 2 x 1 sqrt = 4 in
-    Advance.  A different count means the toolchain fused (or split) something: fail here, on the CPU."""
+    """The fp32 band kernels evaluate one item (4 cells) per lane as two packed pairs: FADD2 / FMUL2 / FFMA2.
+    ptxas 12.9 contracts mul.rn.f32x2 + add.rn.f32x2 into one FFMA2 even under -fmad=false, which would break
+    the arithmetic contract (R18: no FMA contraction); ls_math.cuh forms every product that feeds a sum as
+    fma(a, b, +0) to prevent it.  The packed instruction mix per kernel is therefore fixed by the formulas:
+      reinit sweep, per pair: 6 differences + 5 sums + den^2 + 2 sqrt seeds + (g - 1) + (c - dtau U) = 16 FADD2;
+        6 scalings + 2x2 sqrt + U = 11 FMUL2; 6 squares + 2 (den^2) + 2x2 sqrt + 5 divide + dtau U = 18 FFMA2
+      Advance, per pair: 16 FADD2, 13 FMUL2, 10 FFMA2
+    and two pairs per item.  A different count means the toolchain fused (or split) something: fail here, on
+    the CPU.  (The scalar slow path of the same kernels uses FADD / FMUL / FFMA, which are not counted.)"""
     import re
     import shutil
     import subprocess
@@ -105,16 +108,21 @@ def test_packed_fp32_arithmetic_is_not_contracted():
         if m:
             fn = m.group(1)
             continue
-        if fn and "FFMA2" in line:
-            counts[fn] = counts.get(fn, 0) + 1
-        if fn and ("UTMALDG" in line or "UBLKCP" in line):
+        if not fn:
+            continue
+        for op in ("FFMA2", "FMUL2", "FADD2"):
+            if re.search(r"\b" + op + r"\b", line):
+                counts.setdefault(fn, {}).setdefault(op, 0)
+                counts[fn][op] += 1
+        if "UTMALDG" in line or "UBLKCP" in line:
             tma_ops[fn] = tma_ops.get(fn, 0) + 1
-    reinit_f32 = [f for f in counts if "k_reinit_tmaIf" in f]
-    advance_f32 = [f for f in counts if "k_advance_tmaIf" in f]
+    # mangled: k_band_tile<float, ADV, SWEEPS, ...> -> "k_band_tileIfLb0ELi1E..." (reinit) / "k_band_tileIfLb1ELi0E..." (advance)
+    reinit_f32 = [f for f in counts if "k_band_tileIfLb0ELi1E" in f]
+    advance_f32 = [f for f in counts if "k_band_tileIfLb1ELi0E" in f]
     assert len(reinit_f32) == 5 and len(advance_f32) == 1, (reinit_f32, advance_f32)
     for f in reinit_f32:
-        assert counts[f] == 18, (f, counts[f])
-    assert counts[advance_f32[0]] == 4, counts[advance_f32[0]]
+        assert counts[f] == {"FFMA2": 36, "FMUL2": 22, "FADD2": 32}, (f, counts[f])
+    assert counts[advance_f32[0]] == {"FFMA2": 20, "FMUL2": 26, "FADD2": 32}, counts[advance_f32[0]]
     # and the band kernels really are TMA kernels (cp.async.bulk.tensor -> UTMALDG, cp.async.bulk -> UBLKCP)
     for f in reinit_f32 + advance_f32:
         assert tma_ops.get(f, 0) >= 2, f
