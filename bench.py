@@ -57,6 +57,8 @@ def parse_args():
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (1-based); bench line = 4")
     ap.add_argument("--n", type=int, default=None, help="grid edge override (smoke runs of the bench itself)")
     ap.add_argument("--rebuild", default="incremental", choices=["incremental", "full"])
+    ap.add_argument("--fuse", type=int, default=0, choices=[0, 1, 2],
+                    help="reinit sweeps per launch: 0 = library default (2), 1 = no temporal blocking, 2")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -225,8 +227,8 @@ def run_ours(args):
     d_F = h_F.cuda(non_blocking=True)
     stream = torch.cuda.current_stream()
     ctx = ls.ls_create(w.nx, w.ny, w.nz, ls.LS_F32 if esz == 4 else ls.LS_F64, stream.cuda_stream)
-    p0 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild, 0)
-    p1 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild, 1)
+    p0 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild, 0, args.fuse)
+    p1 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild, 1, args.fuse)
     out = {}
     try:
         # ---- warm-up (unchained: resync copy + whole-grid scan + global clamp happen here, once) ----

@@ -33,7 +33,7 @@ SYMBOLS = (
 class ls_params(C.Structure):
     _fields_ = [("dx", C.c_double), ("dt", C.c_double), ("dtau", C.c_double), ("beta", C.c_double),
                 ("gamma", C.c_double), ("iters", C.c_int32), ("rebuild", C.c_int32),
-                ("chained", C.c_int32), ("reserved", C.c_int32)]
+                ("chained", C.c_int32), ("fuse", C.c_int32)]
 
 
 class LsError(RuntimeError):
@@ -163,8 +163,8 @@ def ls_reinit_tol(ctx: int, d, phi_bar, dtau: float, dx: float, gamma: float, to
     return k.value, r.value, st == LS_OK
 
 
-def make_params(dx, dt, dtau, beta, gamma, iters, rebuild=LS_REBUILD_FULL, chained=0) -> ls_params:
-    return ls_params(dx, dt, dtau, beta, gamma, iters, rebuild, chained, 0)
+def make_params(dx, dt, dtau, beta, gamma, iters, rebuild=LS_REBUILD_FULL, chained=0, fuse=0) -> ls_params:
+    return ls_params(dx, dt, dtau, beta, gamma, iters, rebuild, chained, fuse)
 
 
 def ls_step(ctx: int, phi, F, p: ls_params, n_steps: int) -> None:

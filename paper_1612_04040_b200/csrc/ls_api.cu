@@ -225,10 +225,16 @@ ls_status step_impl(ls_ctx* c, T* phi, const T* F, const ls_params* p, int n_ste
         T* src = S;
         T* dst = phi;
         bool emitted = false;
-        for (int it = 0; it < p->iters; ++it) {                                     // Step 3
-            const bool last = it == p->iters - 1 && dst == phi;
+        // Step 3: `iters` sweeps in launches of 2 (temporal blocking, tile path only) or 1.  The number of
+        // launches should be odd so that the last one lands in phi; if it cannot be (iters == 0, or an even
+        // count on the scalar path), the band copy below moves the result.
+        const bool can_fuse = p->fuse != 1 && ls::tile_usable<T>(c->g, phi, S, (const void*)nullptr);
+        int pairs = can_fuse ? p->iters / 2 : 0, singles = p->iters - 2 * pairs;
+        if (pairs > 0 && ((pairs + singles) & 1) == 0) { pairs -= 1; singles += 2; }
+        for (int l = 0; l < pairs + singles; ++l) {
+            const bool last = l == pairs + singles - 1 && dst == phi;
             ls::BandOp r;
-            r.sweeps = 1;
+            r.sweeps = l < pairs ? 2 : 1;
             r.list = c->bb.lb;
             r.clamp = last;
             r.emit_T = last && incremental;
@@ -265,7 +271,7 @@ ls_status check_step_args(ls_ctx* c, const void* phi, const void* F, const ls_pa
     if (n_steps < 0 || p->iters < 0) return LS_ERR_ARG;
     if (!(p->dx > 0) || !(p->beta > 0) || !(p->beta < p->gamma) || std::isinf(p->gamma)) return LS_ERR_ARG;
     if (p->rebuild != LS_REBUILD_FULL && p->rebuild != LS_REBUILD_INCREMENTAL) return LS_ERR_ARG;
-    if ((p->chained != 0 && p->chained != 1) || p->reserved != 0) return LS_ERR_ARG;
+    if ((p->chained != 0 && p->chained != 1) || p->fuse < 0 || p->fuse > 2) return LS_ERR_ARG;
     return LS_OK;
 }
 
@@ -327,10 +333,12 @@ ls_status ls_create(int32_t nx, int32_t ny, int32_t nz, ls_dtype dtype, void* cu
         alloc((void**)&bb.qflagN[i], nq + 16, true);          // invariant: 1 exactly at the quads of qlist[i]
         alloc((void**)&bb.items[i], nq * ls::kItemsPerQuad * sizeof(uint16_t), false);
         alloc((void**)&bb.qlist[i], nq * sizeof(ls::QuadEntry), false);
+        alloc((void**)&bb.qneed[i], nq * ls::kNeedBytes, false);
     }
     alloc((void**)&bb.nmask, nq * 32 * sizeof(uint64_t), true);   // invariant: zero outside the band last built
     alloc((void**)&bb.qcount, nq * sizeof(int32_t), true);
     alloc((void**)&bb.partials, 1024 * sizeof(int32_t), true);
+    alloc((void**)&bb.zero_page, 256, true);
     alloc((void**)&bb.counts, sizeof(ls::Counts), true);
     alloc((void**)&c->residual, 8, true);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&c->host_counts, sizeof(ls::Counts));
@@ -351,7 +359,7 @@ ls_status ls_destroy(ls_ctx* c) {
     cudaStreamSynchronize(c->stream);
     ls::BandBuffers& bb = c->bb;
     void* dev[] = {bb.tmask[0], bb.tmask[1], bb.qflagT[0], bb.qflagT[1], bb.qflagN[0], bb.qflagN[1], bb.items[0], bb.items[1],
-                   bb.qlist[0], bb.qlist[1], bb.nmask, bb.qcount, bb.partials, bb.counts, bb.ex_cnt, bb.T_ids, bb.N_ids,
+                   bb.qlist[0], bb.qlist[1], bb.qneed[0], bb.qneed[1], bb.nmask, bb.qcount, bb.partials, bb.zero_page, bb.counts, bb.ex_cnt, bb.T_ids, bb.N_ids,
                    bb.T_masks, bb.N_masks, c->residual, c->scratch, c->dev_phi, c->dev_F, c->snap[0], c->snap[1]};
     for (void* p : dev)
         if (p) cudaFree(p);

@@ -107,6 +107,7 @@ struct DilateArgs {
     uint8_t* qflagN;           // out: flags of the band being built
     int32_t* qcount;           // out: items per quad
     uint16_t* items;           // out: item lists
+    uint8_t* qneed;            // out: load maps
     Counts* counts;
 };
 
@@ -273,7 +274,72 @@ __global__ void __launch_bounds__(kDilateWarps * 32) k_dilate_items(Geom g, Dila
         const int pieces = (total + 7) >> 3;
         for (int i = lane; i < pieces; i += 32) dst[i] = src[i];
     }
-    if (lane == 0) { a.qflagN[c] = total ? 1 : 0; a.qcount[c] = total; }
+    // Load map (kNeedBytes, ls_internal.h): a chunk is needed if an N point of the quad reads one of its cells:
+    // its own chunk, the same chunk one row up / down in y or z, or — for a point in the first / last cell of a
+    // chunk — the chunk next to it in x.  Pieces outside the domain are never needed (edge replicate patches them).
+    // Lane (j, lz) reduces its word to three 8-bit masks over y: R = rows of brick j, layer lz that hold an N point,
+    // E0 / E7 = rows whose first / last cell is one; the needs of the chunks of brick j in layer lz are then
+    // D = R | R<<1 | R>>1 | R(lz-1) | R(lz+1) | E7(j-1) | E0(j+1), and a transposition through shared memory
+    // turns the per-(j, lz) masks over y into the per-row bytes over chunks.
+    {
+        auto gather = [](uint64_t m) -> unsigned {   // bit 0 of each byte -> one 8-bit mask
+            return (unsigned)(((m & COL0) * 0x0102040810204080ull) >> 56);
+        };
+        uint64_t f = n | (n >> 4);
+        f |= f >> 2;
+        f |= f >> 1;
+        const unsigned R = gather(f), E0 = gather(n), E7 = gather(n >> 7);
+        const unsigned Rdn = __shfl_up_sync(0xffffffffu, R, 1), Rup = __shfl_down_sync(0xffffffffu, R, 1);
+        const unsigned E7l = __shfl_up_sync(0xffffffffu, E7, 8), E0r = __shfl_down_sync(0xffffffffu, E0, 8);
+        unsigned D = R | ((R << 1) & 0xffu) | (R >> 1);
+        if (lz > 0) D |= Rdn;
+        if (lz < 7) D |= Rup;
+        if (j > 0) D |= E7l;
+        if (j < 3) D |= E0r;
+        __syncwarp();   // s_words (read as `sb` above) is reused as the transposition buffer
+        unsigned char* tb = reinterpret_cast<unsigned char*>(s_words[wib]);   // [0,32) D(j,lz)  [32,64) R(j,lz)  [64,72) E0(0,lz)  [72,80) E7(3,lz)
+        tb[lane] = (unsigned char)D;
+        tb[32 + lane] = (unsigned char)R;
+        if (j == 0) tb[64 + lz] = (unsigned char)E0;
+        if (j == 3) tb[72 + lz] = (unsigned char)E7;
+        __syncwarp();
+        uint8_t* need_out = a.qneed + (int64_t)c * kNeedBytes;
+        for (int r = lane; r < 100; r += 32) {
+            const int y = r % 10 - 1, z = r / 10 - 1;
+            const bool yin = y >= 0 && y < 8, zin = z >= 0 && z < 8;
+            unsigned need = 0;
+            if (yin && zin) {
+#pragma unroll
+                for (int jj = 0; jj < 4; ++jj) need |= (((unsigned)tb[jj * 8 + z] >> y) & 1u) << (1 + jj);
+                need |= ((unsigned)tb[64 + z] >> y) & 1u;
+                need |= (((unsigned)tb[72 + z] >> y) & 1u) << 5;
+            } else if (zin) {   // a halo row in y: read by the quad row next to it
+#pragma unroll
+                for (int jj = 0; jj < 4; ++jj) need |= (((unsigned)tb[32 + jj * 8 + z] >> (y < 0 ? 0 : 7)) & 1u) << (1 + jj);
+            } else if (yin) {   // a halo row in z (corner rows are never read)
+#pragma unroll
+                for (int jj = 0; jj < 4; ++jj) need |= (((unsigned)tb[32 + jj * 8 + (z < 0 ? 0 : 7)] >> y) & 1u) << (1 + jj);
+            }
+            const int gy = by * 8 + y, gz = bz * 8 + z;
+            if (gy < 0 || gy >= g.ny || gz < 0 || gz >= g.nz) need = 0;
+            if (qx == 0) need &= ~1u;
+#pragma unroll
+            for (int ch = 0; ch < 5; ++ch)
+                if (qx * 32 + ch * 8 >= g.nx) need &= ~(2u << ch);
+            need_out[r] = (uint8_t)need;
+        }
+        for (int r = lane; r < 64; r += 32) {
+            const int y = r & 7, z = r >> 3;
+            unsigned own = 0;
+#pragma unroll
+            for (int jj = 0; jj < 4; ++jj) own |= (((unsigned)tb[32 + jj * 8 + z] >> y) & 1u) << jj;
+            need_out[112 + r] = (uint8_t)own;
+        }
+    }
+    // does an N point sit on the quad's low-x / high-x face?  (the band kernels load that x halo only then)
+    const unsigned faceL = __ballot_sync(0xffffffffu, j == 0 && (n & COL0) != 0);
+    const unsigned faceR = __ballot_sync(0xffffffffu, j == 3 && (n & COL7) != 0);
+    if (lane == 0) { a.qflagN[c] = total ? 1 : 0; a.qcount[c] = total | (faceL ? 1 << 16 : 0) | (faceR ? 1 << 17 : 0); }
     }   // quads of this turn
     }   // turns
 }
@@ -510,6 +576,7 @@ void launch_build_lists(const Geom& g, BandBuffers& bb, bool incremental, int it
     a.qflagN = bb.qflagN[cr];
     a.qcount = bb.qcount;
     a.items = bb.items[cr];
+    a.qneed = bb.qneed[cr];
     a.counts = bb.counts;
     // Persistent warps: the candidate count lives on the device (ls_step never synchronises).
     const unsigned blocks = (unsigned)(sm_count() * 8);

@@ -31,12 +31,18 @@ struct Geom {
 };
 
 constexpr int kItemsPerQuad = 512;   // 64 rows x 8 groups of 4 cells
+// Load map of a quad's tile (one-sweep band kernels): which 32-byte brick rows ("chunks") of the 10 x 10 tile
+// rows hold a cell that some N point of the quad reads — the band kernels fetch only those.
+//   [0, 100)    need byte of tile row rz*10 + ry (rz = z + 1, ry = y + 1): bit 0 = the x-halo piece left of the
+//               quad, bits 1..4 = chunks 0..3 of the quad, bit 5 = the x-halo piece right of it
+//   [112, 176)  own byte of quad row z*8 + y: bit j = brick j has an N point in that row (Advance reads F there)
+constexpr int kNeedBytes = 176;
 constexpr int kTickets = 16;
 
 // One entry of a quad list.
 struct QuadEntry {
     int32_t quad;    // quad id
-    int32_t nitems;  // items in its list (1..512)
+    int32_t nitems;  // items in its list (1..512) | x-face flags, see BandBuffers::qcount
 };
 
 // Device-resident counters, written by the band builder, read by the band kernels (so the host
@@ -62,7 +68,10 @@ struct BandBuffers {
     uint64_t* nmask;      // [nquads*32] N mask words of the band last built; all-zero for quads outside N
     uint8_t* qflagN[2];   // [nquads] quad holds an N point, per list buffer
     uint16_t* items[2];   // [nquads*512] item lists, dense by quad id, per list buffer
-    int32_t* qcount;      // [nquads] items of the quad in the band being built
+    uint8_t* qneed[2];    // [nquads*kNeedBytes] load maps, dense by quad id, per list buffer
+    int32_t* qcount;      // [nquads] items of the quad in the band being built (bits 0-15) | N point on the quad's
+                          // low-x face (bit 16) / high-x face (bit 17): the band kernels load that x halo only then
+    void* zero_page;      // 256 zero bytes
     QuadEntry* qlist[2];  // [nquads] N quad list per list buffer
     int32_t* partials;    // [<= 1024] per-CTA counts of k_compact
     Counts* counts;

@@ -1,20 +1,25 @@
 // ls_tile.cu — the band kernels of Steps 2 and 3: persistent, warp-specialised, TMA-fed.
 //
-// Tile = one QUAD (four x-adjacent 8^3 bricks, 32 x 8 x 8 points; ls_internal.h) plus a halo of K cells in
-// y and z and of one 16-byte piece in x (fp32: 4 cells, fp64: 2), K = number of operations fused in the
-// launch (Advance and / or reinit sweeps: temporal blocking).  Every tile row is
-// 160 (fp32) / 288 (fp64) contiguous bytes of a field row that starts 16 bytes before a 128-byte line.
+// Tile = one QUAD (four x-adjacent 8^3 bricks, 32 x 8 x 8 points; ls_internal.h).  In shared memory:
+//   M  [8+2K][8+2K][32]   the quad and K halo rows in y and z: every row is one aligned 128-byte line (fp32)
+//   L, R [6+2K][6+2K][XW] the x halo, one 16-byte piece per row (fp32: 4 cells, fp64: 2), loaded only when an
+//                         N point sits on that edge of the quad (K = 1) — a third of the sectors otherwise
+// K = number of operations fused in the launch: K = 1 is Advance or one reinit sweep; K = 2 is two sweeps
+// (temporal blocking of eq. 12's pseudo-time iterations): sweep 1 is evaluated on the
+// quad's N points AND on the N points of the one-cell ring around it (neighbour quads' masks), kept in
+// registers until every read of iteration k is done, written back IN PLACE, and sweep 2 then runs on the
+// quad's own points.  Jacobi order is preserved exactly, so K = 2 equals two K = 1 launches bit for bit.
 //
 //   producer warp (one elected lane)   takes quads from the ordered quad list through a device ticket
-//        counter (chunks of 4), and per quad issues ONE cp.async.bulk.tensor.3d box load of the halo tile
+//        counter (chunks of 4), and per quad issues up to three cp.async.bulk.tensor.3d box loads (M, L, R)
 //        straight from the dense x-fastest field, one cp.async.bulk of the quad's
-//        precomputed item list (and, for Advance, the 32x8x8 box of F and the quad's 32 T mask words), all
-//        completing on the stage's "full" mbarrier; it waits on the stage's "empty" mbarrier before reuse.
-//   4 consumer warps   wait on "full"; edge-replicate the out-of-domain halo (R3; TMA zero-fills it);
-//        lane l evaluates items l, l+128, ...: one item = 4 x-consecutive cells = 5 LDS.128 + 2 LDS.32,
-//        two packed fp32 pairs through eq. 3-8 / eq. 12-13 (ls_math.cuh), one 16-byte store — Jacobi: reads
-//        come from the tile, results go to the other global buffer (K = 1) or to the second tile buffer
-//        (K > 1).  No CTA barrier per tile: each warp arrives on "empty" when it is done with the stage.
+//        precomputed item list (Advance: the 32x8x8 box of F and the quad's 32 T mask words; K = 2: the N
+//        masks of the six neighbour quads), all completing on the stage's "full" mbarrier; it waits on the
+//        stage's "empty" mbarrier before reuse.
+//   consumer warps   wait on "full"; edge-replicate the out-of-domain halo (R3; TMA zero-fills it); lane l
+//        evaluates items l, l+NC, ...: one item = 4 x-consecutive cells = 5 LDS.128 + 2 LDS.32, two packed
+//        fp32 pairs through eq. 3-8 / eq. 12-13 (ls_math.cuh), one 16-byte store to the other global buffer.
+//        K = 1 needs no CTA barrier per tile: each warp arrives on "empty" when it is done with the stage.
 // The arithmetic is bit-identical to the scalar kernels of ls_stencil.cu, which remain the path for grids the
 // tile path cannot address (nx not a multiple of 4, unaligned fields).
 #include <cuda.h>
@@ -26,14 +31,7 @@ namespace ls {
 
 namespace {
 
-constexpr int kConsumerWarps = 4;
-constexpr int kConsumers = kConsumerWarps * 32;
-constexpr int kThreads = kConsumers + 32;   // + the producer warp
 constexpr int kChunk = 4;                   // quads per ticket
-
-template <typename T> struct XHalo;
-template <> struct XHalo<float> { static constexpr int XH = 4; };
-template <> struct XHalo<double> { static constexpr int XH = 2; };
 
 constexpr int round128(int x) { return (x + 127) / 128 * 128; }
 
@@ -45,25 +43,30 @@ struct alignas(16) Hdr {
     int edge;       // tile reaches outside the domain (halo needs patching)
     long long org;  // element offset of the first cell in the dense field
     int tvalid;     // Advance: T masks were loaded (else the quad holds no T point)
-    int pad;
+    int ring_n;     // K = 2: entries of the ring list (consumers count them up from 0)
+    int haveL, haveR;   // the x halo pieces were loaded
 };
 
 // One pipeline stage in shared memory.
 template <typename T, int K, bool ADV>
 struct Stage {
-    static constexpr int XH = XHalo<T>::XH;
-    static constexpr int PX = 32 + 2 * XH;
+    static constexpr int XW = 16 / (int)sizeof(T);
     static constexpr int PY = 8 + 2 * K;
-    static constexpr int ELEMS = PX * PY * PY;
-    static constexpr int TILE_BYTES = ELEMS * (int)sizeof(T);
-    static constexpr int OFF_TILE2 = round128(TILE_BYTES);                       // second tile buffer (K > 1)
-    static constexpr int OFF_F = OFF_TILE2 + (K > 1 ? round128(TILE_BYTES) : 0);
+    static constexpr int PH = 6 + 2 * K;
+    static constexpr int M_BYTES = PY * PY * 32 * (int)sizeof(T);
+    static constexpr int H_BYTES = PH * PH * 16;
+    static constexpr int OFF_L = round128(M_BYTES);
+    static constexpr int OFF_R = OFF_L + round128(H_BYTES);
+    static constexpr int OFF_F = OFF_R + round128(H_BYTES);
     static constexpr int F_BYTES = ADV ? 2048 * (int)sizeof(T) : 0;
     static constexpr int OFF_ITEMS = OFF_F + F_BYTES;
-    static constexpr int ITEM_BYTES = kItemsPerQuad * 2;
-    static constexpr int OFF_TM = OFF_ITEMS + ITEM_BYTES;
+    static constexpr int OFF_TM = OFF_ITEMS + kItemsPerQuad * 2;
     static constexpr int TM_BYTES = ADV ? 256 : 0;
-    static constexpr int OFF_HDR = OFF_TM + TM_BYTES;
+    static constexpr int OFF_NB = OFF_TM + TM_BYTES;            // K = 2: y-, y+, z-, z+ quads (256 B each), left quad's
+    static constexpr int NB_BYTES = K > 1 ? 4 * 256 + 2 * 64 : 0;   // brick 3 and right quad's brick 0 (64 B each)
+    static constexpr int OFF_RING = OFF_NB + NB_BYTES;
+    static constexpr int RING_BYTES = K > 1 ? 256 * 4 : 0;
+    static constexpr int OFF_HDR = OFF_RING + RING_BYTES;
     static constexpr int BYTES = round128(OFF_HDR + (int)sizeof(Hdr));
     static_assert(sizeof(Hdr) <= 64, "header slot");
 };
@@ -94,7 +97,8 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kConsumers) : "memory"); }
+template <int NC>
+__device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, %0;" ::"n"(NC) : "memory"); }
 
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int x, int y, int z) {
     asm volatile(
@@ -102,35 +106,71 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
         "l"(map), "r"(bar), "r"(x), "r"(y), "r"(z)
         : "memory");
 }
+// 16-byte asynchronous copy global -> shared (LDGSTS, L2 only), and the arrive that fires when all of this
+// thread's earlier ones have landed (the barrier's expected count includes it: .noinc).
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_arrive(uint32_t bar) {
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+}
 __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
                  "l"(src), "r"(bytes), "r"(bar)
                  : "memory");
 }
 
+// The three arrays of a tile.  Coordinates are relative to the quad's first cell.
+template <typename T, int K>
+struct Tile {
+    static constexpr int XW = 16 / (int)sizeof(T), PY = 8 + 2 * K, PH = 6 + 2 * K;
+    T* M;
+    T* L;
+    T* R;
+    // offset in M of cell (x, y, z), x in [0, 32), y, z in [-K, 8 + K)
+    __device__ __forceinline__ static int om(int x, int y, int z) { return ((z + K) * PY + (y + K)) * 32 + x; }
+    // offset in L / R of column c of row (y, z), y, z in [-(K-1), 8 + K - 1)
+    __device__ __forceinline__ static int oh(int c, int y, int z) { return ((z + K - 1) * PH + (y + K - 1)) * XW + c; }
+    // any cell of the tile's cover: x in [-XW, 32 + XW) (x outside [0, 32) only for rows L / R hold)
+    __device__ __forceinline__ T& at(int x, int y, int z) const {
+        if (x < 0) return L[oh(x + XW, y, z)];
+        if (x >= 32) return R[oh(x - 32, y, z)];
+        return M[om(x, y, z)];
+    }
+};
+
 // R3: TMA zero-fills cells outside the domain; give them the value of the nearest in-domain cell (edge
 // replicate).  Sources are in-domain cells, destinations are not: no ordering needed inside.  Only called for
-// tiles that reach outside the domain (uniform over the consumers).  `tile` may be either tile buffer.
-template <typename T, int PX, int PY, int XH, int K>
-__device__ __noinline__ void patch_boundary(T* tile, const Geom& g, int x0, int y0, int z0, int ctid) {
-    const int ox = x0 - XH, oy = y0 - K, oz = z0 - K;
-    for (int e = ctid; e < PX * PY * PY; e += kConsumers) {
-        const int x = e % PX, r = e / PX, y = r % PY, z = r / PY;
-        const int gx = ox + x, gy = oy + y, gz = oz + z;
+// tiles that reach outside the domain (uniform over the consumers).  Ends with a consumer barrier.
+template <typename T, int K, int NC>
+__device__ __noinline__ void patch_boundary(const Tile<T, K>& t, const Geom& g, int x0, int y0, int z0, int ctid) {
+    constexpr int XW = Tile<T, K>::XW, PY = Tile<T, K>::PY, PH = Tile<T, K>::PH;
+    auto fix = [&](int x, int y, int z) {
+        const int gx = x0 + x, gy = y0 + y, gz = z0 + z;
         const int cx = min(max(gx, 0), g.nx - 1), cy = min(max(gy, 0), g.ny - 1), cz = min(max(gz, 0), g.nz - 1);
         if (cx != gx || cy != gy || cz != gz) {
-            const int sx = cx - ox, sy = cy - oy, sz = cz - oz;
-            if (sx >= 0 && sx < PX && sy >= 0 && sy < PY && sz >= 0 && sz < PY) tile[e] = tile[(sz * PY + sy) * PX + sx];
+            const int sx = cx - x0, sy = cy - y0, sz = cz - z0;
+            // the nearest in-domain cell lies in the tile's cover unless the tile misses the domain in x by more
+            // than its halo (cannot happen: a listed quad holds in-domain cells)
+            if (sx >= -XW && sx < 32 + XW) t.at(x, y, z) = t.at(sx, sy, sz);
         }
+    };
+    for (int e = ctid; e < PY * PY * 32; e += NC) fix(e & 31, (e >> 5) % PY - K, (e >> 5) / PY - K);
+    for (int e = ctid; e < PH * PH * XW * 2; e += NC) {
+        const int side = e / (PH * PH * XW), r = e % (PH * PH * XW);
+        const int c = r % XW, row = r / XW;
+        fix(side ? 32 + c : c - XW, row % PH - (K - 1), row / PH - (K - 1));
     }
     fence_proxy_async();   // generic writes into a tile a later TMA load overwrites
-    consumer_sync();
+    consumer_sync<NC>();
 }
 
-// The stencil of the item whose first cell sits at tile offset o.
-template <typename T, int PX, int PY>
-__device__ __forceinline__ void load_item(const T* tile, int o, Item4<T>& s) {
-    constexpr int SY = PX, SZ = PX * PY;
+// The stencil of the item at group xq (0..7) of row (y, z) of the quad.
+template <typename T, int K>
+__device__ __forceinline__ void load_item(const Tile<T, K>& t, int xq, int y, int z, Item4<T>& s) {
+    constexpr int SY = 32, SZ = 32 * Tile<T, K>::PY, XW = Tile<T, K>::XW;
+    const int o = Tile<T, K>::om(xq * 4, y, z);
+    const T* tile = t.M;
     if (sizeof(T) == 4) {
         union V { float4 q; T e[4]; } c, ym, yp, zm, zp;
         c.q = *reinterpret_cast<const float4*>(tile + o);
@@ -153,8 +193,11 @@ __device__ __forceinline__ void load_item(const T* tile, int o, Item4<T>& s) {
 #pragma unroll
         for (int e = 0; e < 4; ++e) { s.c[e] = c.e[e]; s.ym[e] = ym.e[e]; s.yp[e] = yp.e[e]; s.zm[e] = zm.e[e]; s.zp[e] = zp.e[e]; }
     }
-    s.xm = tile[o - 1];
-    s.xp = tile[o + 4];
+    const int h = Tile<T, K>::oh(0, y, z);
+    const T* pm = xq > 0 ? tile + o - 1 : t.L + h + XW - 1;
+    const T* pp = xq < 7 ? tile + o + 4 : t.R + h;
+    s.xm = *pm;
+    s.xp = *pp;
 }
 template <typename T>
 __device__ __forceinline__ void store4(T* p, const T v[4]) {
@@ -170,28 +213,35 @@ struct TileArgs {
     const QuadEntry* qlist;
     const int32_t* count;
     const uint16_t* items;
+    const uint8_t* qneed;         // K = 1: load maps (ls_internal.h)
+    const uint64_t* nmask;        // K = 2: N masks of the band (zero for quads outside it)
+    const void* zero_page;        // 256 zero bytes (neighbour quads outside the domain)
     const uint64_t* tmask_in;     // Advance: T masks of the band (tmask[tb])
     const uint8_t* qflagT_in;
     const uint8_t* tgate;         // null or validity gate of tmask_in
     uint64_t* tmask_out;          // EMIT_T: tmask[tb ^ 1]
     uint8_t* qflagT_out;
     unsigned long long* residual;
+    const void* src;              // K = 1: the field the tiles are gathered from, and F (Advance)
+    const void* F;
     unsigned int* ticket;         // [0] next list index, [1] CTAs done (self-resetting)
-    int reverse;                  // walk the list from its end (L2 reuse between consecutive sweeps)
+    int reverse;                  // walk the list from its end
 };
 
 // ---------------------------------------------------------------------------------------------
-// One launch = (ADV ? Advance : nothing) followed by SWEEPS reinit sweeps on every listed quad, K = ADV + SWEEPS
-// operations deep, results of the last operation written to `dst` at the item cells.
+// One launch = Advance (ADV, K = 1), or K reinit sweeps, on every listed quad; results of the last operation
+// are written to `dst` at the item cells.  NCW consumer warps + 1 producer warp.
 // ---------------------------------------------------------------------------------------------
-template <typename T, bool ADV, int SWEEPS, bool CLAMP, bool RESIDUAL, bool EMIT_T, int STAGES>
-__global__ void __launch_bounds__(kThreads)
-k_band_tile(const __grid_constant__ CUtensorMap tm_src, const __grid_constant__ CUtensorMap tm_F, T* __restrict__ dst,
-            Geom g, StencilParams<T> pa, StencilParams<T> pr, TileArgs a) {
-    constexpr int K = (ADV ? 1 : 0) + SWEEPS;
-    static_assert(K == 1, "temporal blocking (K > 1) is built by k_band_tile_multi");
+template <typename T, bool ADV, int K, bool CLAMP, bool RESIDUAL, bool EMIT_T, int STAGES, int NCW, int NPW>
+__global__ void __launch_bounds__((NCW + NPW) * 32)
+k_band_tile(const __grid_constant__ CUtensorMap tm_M, const __grid_constant__ CUtensorMap tm_H,
+            const __grid_constant__ CUtensorMap tm_F, T* __restrict__ dst, Geom g, StencilParams<T> pa,
+            StencilParams<T> pr, TileArgs a) {
+    static_assert(K == 1 || (K == 2 && !ADV && NCW == 8 && NPW == 1), "K = 2: two reinit sweeps, 256 consumers");
+    static_assert(K != 1 || NPW == STAGES, "K = 1: one producer warp per stage");
     using S = Stage<T, K, ADV>;
-    constexpr int PX = S::PX, PY = S::PY, XH = S::XH;
+    using TL = Tile<T, K>;
+    constexpr int NC = NCW * 32, XW = S::XW;
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t smem_base = smem_u32(smem);
@@ -200,45 +250,214 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_src, const __grid_constant__ 
     const uint32_t bar_full = smem_base + STAGES * S::BYTES + 512, bar_empty = bar_full + 8 * STAGES;
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < STAGES; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, kConsumerWarps); }
+        for (int s = 0; s < STAGES; ++s) { mbar_init(bar_full + 8 * s, K == 1 ? 33 : 1); mbar_init(bar_empty + 8 * s, NCW); }
         fence_barrier_init();
     }
     if (EMIT_T && tid < 128) tstage[tid] = 0u;
+    // K = 1 fetches only the chunks its items read; the rest of a stage keeps what earlier tiles left there, which
+    // only feeds results that are thrown away (cells of an item outside N).  Start from zeros, not from whatever
+    // bit patterns the last kernel left in shared memory (a NaN would send a lane down the scalar slow path).
+    for (int i = tid; i < STAGES * S::BYTES / 16; i += (NCW + NPW) * 32) reinterpret_cast<uint4*>(smem)[i] = make_uint4(0u, 0u, 0u, 0u);
     __syncthreads();
     const int count = *a.count;
 
-    if (warp == kConsumerWarps) {
-        // ------------------------------ producer ------------------------------
+    if (warp >= NCW && K == 1) {
+        // ------------------------------ producer, K = 1: sparse gather ------------------------------
+        // The whole warp works.  Lane pair (2s, 2s+1) owns tile rows s, s+16, ..., s+96 (of 10 x 10): per needed
+        // chunk of a row each lane of the pair copies one 16-byte half with cp.async (the two halves of a 32-byte
+        // sector leave in one instruction and coalesce into one sector request); lane 2s also copies the row's left
+        // x-halo piece, lane 2s+1 the right one.  Which chunks: the load map the band builder wrote (kNeedBytes).
+        // One producer warp per stage: warp p fills stage p only, with tiles it draws itself from the ticket counter,
+        // so it has STAGES tile periods for each tile it issues.
+        constexpr int NPASS = 7;
+        const int half = lane & 1, rslot = lane >> 1;
+        const T* src = reinterpret_cast<const T*>(a.src);
+        const T* Fsrc = reinterpret_cast<const T*>(a.F);
+        struct Need { uint32_t lo, hi, own; };   // need bytes of passes 0-3, 4-6; own nibbles of the 4 F passes
+        auto load_entry = [&](int idx) -> QuadEntry {
+            QuadEntry e;
+            e.quad = -1; e.nitems = 0;
+            if (idx >= 0) e = a.qlist[a.reverse ? count - 1 - idx : idx];
+            return e;
+        };
+        auto load_need = [&](int quad) -> Need {
+            Need n;
+            n.lo = n.hi = n.own = 0;
+            if (quad >= 0) {
+                const uint8_t* nd = a.qneed + (int64_t)quad * kNeedBytes;
+                n.lo = (uint32_t)nd[rslot] | ((uint32_t)nd[rslot + 16] << 8) | ((uint32_t)nd[rslot + 32] << 16) |
+                       ((uint32_t)nd[rslot + 48] << 24);
+                n.hi = (uint32_t)nd[rslot + 64] | ((uint32_t)nd[rslot + 80] << 8) |
+                       ((uint32_t)(rslot < 4 ? nd[rslot + 96] : 0) << 16);
+                if (ADV)
+                    n.own = (uint32_t)nd[112 + rslot] | ((uint32_t)nd[112 + 16 + rslot] << 8) |
+                            ((uint32_t)nd[112 + 32 + rslot] << 16) | ((uint32_t)nd[112 + 48 + rslot] << 24);
+            }
+            return n;
+        };
+        // per-lane constants of the 7 passes: element offset of the row from the quad's first cell, byte offset of
+        // the row in M, byte offset of its piece in L / R (quad rows only)
+        int64_t rowoff[NPASS];
+        uint32_t m_off[NPASS], h_off[NPASS];
+#pragma unroll
+        for (int k = 0; k < NPASS; ++k) {
+            const int r = min(rslot + 16 * k, 99), y = r % 10 - 1, z = r / 10 - 1;
+            rowoff[k] = ((int64_t)z * g.ny + y) * g.nx;
+            m_off[k] = (uint32_t)(r * 32 * (int)sizeof(T));
+            h_off[k] = (uint32_t)(((z & 7) * 8 + (y & 7)) * 16);
+        }
+        int64_t frowoff[4];   // Advance: rows of the F box
+#pragma unroll
+        for (int k = 0; k < 4; ++k) frowoff[k] = ((int64_t)((rslot + 16 * k) >> 3) * g.ny + ((rslot + 16 * k) & 7)) * g.nx;
+        // Scheduling is dynamic, one tile per ticket, and nothing is drawn ahead: a warp takes its next ticket right
+        // after it has fired a tile, and the three dependent round trips (ticket, list entry, load map) run while
+        // the consumers work through the other stages.  Tiles cost between 1 and 512 items, so any tile reserved
+        // early is load imbalance at the end of the launch: with tickets drawn in chunks and one chunk ahead, two
+        // thirds of the list were handed out in the first microsecond and the slowest CTA ran 1.4x the mean.
+        const int slot = warp - NCW;
+        const uint32_t st = smem_base + slot * S::BYTES, bar = bar_full + 8 * slot;
+        Hdr* const h = reinterpret_cast<Hdr*>(smem + slot * S::BYTES + S::OFF_HDR);
+        int issued = 0;
+        for (;;) {
+            int idx = 0;
+            if (lane == 0) idx = (int)atomicAdd(a.ticket, 1u);
+            idx = __shfl_sync(0xffffffffu, idx, 0);
+            if (idx >= count) break;
+            const QuadEntry e_cur = load_entry(idx);
+            const Need n_cur = load_need(e_cur.quad);
+            // ---- prepare (the stage is usually still busy: this is hidden behind the wait below) ----
+            const int quad = e_cur.quad;
+            const int qx = quad % g.NQx, rest = quad / g.NQx, by = rest % g.NBy, bz = rest / g.NBy;
+            const int64_t org = g.idx(qx * 32, by * 8, bz * 8);
+            bool tv = false;
+            if (ADV) tv = a.qflagT_in[quad] != 0 && (a.tgate == nullptr || a.tgate[quad] != 0);
+            const int nitems = e_cur.nitems & 0xffff;
+            const uint32_t item_bytes = (uint32_t)((nitems * 2 + 15) & ~15);
+            const int edge = (qx == 0) | (by == 0) | (bz == 0) | (qx * 32 + 32 + XW > g.nx) | (by * 8 + 8 + K > g.ny) |
+                             (bz * 8 + 8 + K > g.nz);
+            const int avail = g.nx - qx * 32;   // cells of this quad's rows that exist (the domain may cut the last quad)
+            const T* qsrc = src + org;
+            const uint16_t* item_src = a.items + (int64_t)quad * kItemsPerQuad;
+            // ---- the stage's previous tenant has been consumed ----
+            if (issued >= 1) mbar_wait(bar_empty + 8 * slot, (uint32_t)((issued - 1) & 1));
+            // ---- fire ----
+            if (lane == 0) {
+                h->quad = quad;
+                h->nitems = nitems;
+                h->x0 = qx * 32; h->y0 = by * 8; h->z0 = bz * 8;
+                h->org = org;
+                h->edge = edge;
+                h->tvalid = tv ? 1 : 0;
+                mbar_expect_tx(bar, item_bytes + (ADV && tv ? 256 : 0));
+                bulk_load(st + S::OFF_ITEMS, item_src, item_bytes, bar);
+                if (ADV && tv) bulk_load(st + S::OFF_TM, a.tmask_in + (int64_t)quad * 32, 256, bar);
+            }
+#pragma unroll
+            for (int k = 0; k < NPASS; ++k) {
+                const uint32_t need = ((k < 4 ? n_cur.lo : n_cur.hi) >> (8 * (k & 3))) & 0xffu;
+                if (need) {
+                    const T* row = qsrc + rowoff[k];
+                    const uint32_t m = st + m_off[k];
+                    if ((need & 1u) && half == 0) cp_async16(st + S::OFF_L + h_off[k], row - XW);
+                    if ((need & 32u) && half == 1) cp_async16(st + S::OFF_R + h_off[k], row + 32);
+#pragma unroll
+                    for (int ch = 0; ch < 4; ++ch)
+                        if (need & (2u << ch)) {
+#pragma unroll
+                            for (int q = 0; q < 4 / XW; ++q) {   // fp32: one 32-byte sector per chunk; fp64: two
+                                const int c0 = ch * 8 + (q * 2 + half) * XW;
+                                if (c0 < avail) cp_async16(m + c0 * (int)sizeof(T), row + c0);
+                            }
+                        }
+                }
+            }
+            if (ADV && tv) {
+                const T* qF = Fsrc + org;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const uint32_t own = (n_cur.own >> (8 * k)) & 0xfu;
+                    const T* row = qF + frowoff[k];
+                    const uint32_t f = st + S::OFF_F + (uint32_t)((rslot + 16 * k) * 32 * (int)sizeof(T));
+#pragma unroll
+                    for (int ch = 0; ch < 4; ++ch)
+                        if (own & (1u << ch)) {
+#pragma unroll
+                            for (int q = 0; q < 4 / XW; ++q) {
+                                const int c0 = ch * 8 + (q * 2 + half) * XW;
+                                if (c0 < avail) cp_async16(f + c0 * (int)sizeof(T), row + c0);
+                            }
+                        }
+                }
+            }
+            cp_async_arrive(bar);
+            ++issued;
+        }
+        // sentinel: this stage gets no more work
+        if (issued >= 1) mbar_wait(bar_empty + 8 * slot, (uint32_t)((issued - 1) & 1));
+        if (lane == 0) {
+            reinterpret_cast<Hdr*>(smem + slot * S::BYTES + S::OFF_HDR)->quad = -1;
+            mbar_expect_tx(bar_full + 8 * slot, 0);
+        }
+        cp_async_arrive(bar_full + 8 * slot);
+        // self-resetting scheduler: the last producer warp to finish fetching zeroes the counters for the next launch
+        if (lane == 0) {
+            __threadfence();
+            if (atomicAdd(a.ticket + 1, 1u) == gridDim.x * NPW - 1) { a.ticket[0] = 0u; a.ticket[1] = 0u; }
+        }
+        return;
+    }
+    if (warp == NCW) {
+        // ------------------------------ producer, K = 2: one elected lane, TMA boxes ------------------------------
         if (lane != 0) return;
         int slot = 0, issued = 0;
         auto acquire = [&]() {   // the stage's previous tenant has been consumed
             if (issued >= STAGES) mbar_wait(bar_empty + 8 * slot, (uint32_t)((issued / STAGES - 1) & 1));
         };
-        auto advance_slot = [&]() { ++issued; slot = slot == STAGES - 1 ? 0 : slot + 1; };
         auto issue = [&](const QuadEntry e) {
             acquire();
             const int quad = e.quad;
             const int qx = quad % g.NQx, rest = quad / g.NQx, by = rest % g.NBy, bz = rest / g.NBy;
             Hdr* h = reinterpret_cast<Hdr*>(smem + slot * S::BYTES + S::OFF_HDR);
+            const int nitems = e.nitems & 0xffff;
+            // K = 1: the x halo is read only by items on that edge (band builder's flags); K = 2: always (ring cells)
+            const bool haveL = K > 1 || ((e.nitems >> 16) & 1), haveR = K > 1 || ((e.nitems >> 17) & 1);
             h->quad = quad;
-            h->nitems = e.nitems;
+            h->nitems = nitems;
             h->x0 = qx * 32; h->y0 = by * 8; h->z0 = bz * 8;
             h->org = g.idx(qx * 32, by * 8, bz * 8);
-            h->edge = (qx == 0) | (by == 0) | (bz == 0) | (qx * 32 + 32 + XH > g.nx) | (by * 8 + 8 + K > g.ny) |
+            h->edge = (qx == 0) | (by == 0) | (bz == 0) | (qx * 32 + 32 + XW > g.nx) | (by * 8 + 8 + K > g.ny) |
                       (bz * 8 + 8 + K > g.nz);
+            h->ring_n = 0;
+            h->haveL = haveL;
+            h->haveR = haveR;
             const uint32_t st = smem_base + slot * S::BYTES, bar = bar_full + 8 * slot;
-            const uint32_t item_bytes = (uint32_t)((e.nitems * 2 + 15) & ~15);
+            const uint32_t item_bytes = (uint32_t)((nitems * 2 + 15) & ~15);
             bool tv = false;
             if (ADV) tv = a.qflagT_in[quad] != 0 && (a.tgate == nullptr || a.tgate[quad] != 0);
             h->tvalid = tv ? 1 : 0;
-            mbar_expect_tx(bar, S::TILE_BYTES + item_bytes + (ADV && tv ? S::F_BYTES + 256 : 0));
-            tma_load_3d(st, &tm_src, bar, h->x0 - XH, h->y0 - K, h->z0 - K);
+            mbar_expect_tx(bar, S::M_BYTES + (haveL ? S::H_BYTES : 0) + (haveR ? S::H_BYTES : 0) + item_bytes +
+                                    (ADV && tv ? S::F_BYTES + 256 : 0) + S::NB_BYTES);
+            tma_load_3d(st, &tm_M, bar, h->x0, h->y0 - K, h->z0 - K);
+            if (haveL) tma_load_3d(st + S::OFF_L, &tm_H, bar, h->x0 - XW, h->y0 - (K - 1), h->z0 - (K - 1));
+            if (haveR) tma_load_3d(st + S::OFF_R, &tm_H, bar, h->x0 + 32, h->y0 - (K - 1), h->z0 - (K - 1));
             bulk_load(st + S::OFF_ITEMS, a.items + (int64_t)quad * kItemsPerQuad, item_bytes, bar);
             if (ADV && tv) {
                 tma_load_3d(st + S::OFF_F, &tm_F, bar, h->x0, h->y0, h->z0);
                 bulk_load(st + S::OFF_TM, a.tmask_in + (int64_t)quad * 32, 256, bar);
             }
-            advance_slot();
+            if (K > 1) {
+                const int syq = g.NQx, szq = g.NQx * g.NBy;
+                const uint64_t* z = reinterpret_cast<const uint64_t*>(a.zero_page);
+                const uint32_t nb = st + S::OFF_NB;
+                bulk_load(nb, by > 0 ? a.nmask + (int64_t)(quad - syq) * 32 : z, 256, bar);
+                bulk_load(nb + 256, by < g.NBy - 1 ? a.nmask + (int64_t)(quad + syq) * 32 : z, 256, bar);
+                bulk_load(nb + 512, bz > 0 ? a.nmask + (int64_t)(quad - szq) * 32 : z, 256, bar);
+                bulk_load(nb + 768, bz < g.NBz - 1 ? a.nmask + (int64_t)(quad + szq) * 32 : z, 256, bar);
+                bulk_load(nb + 1024, qx > 0 ? a.nmask + (int64_t)(quad - 1) * 32 + 24 : z, 64, bar);
+                bulk_load(nb + 1088, qx < g.NQx - 1 ? a.nmask + (int64_t)(quad + 1) * 32 : z, 64, bar);
+            }
+            ++issued;
+            slot = slot == STAGES - 1 ? 0 : slot + 1;
         };
         auto fetch = [&](int base, QuadEntry* e) {
 #pragma unroll
@@ -251,7 +470,7 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_src, const __grid_constant__ 
         while (base < count) {
             const int nbase = (int)atomicAdd(a.ticket, (unsigned)kChunk);
             fetch(nbase, nxt);
-#pragma unroll
+#pragma unroll 1
             for (int i = 0; i < kChunk; ++i)
                 if (base + i < count) issue(cur[i]);
 #pragma unroll
@@ -269,32 +488,131 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_src, const __grid_constant__ 
     }
 
     // ------------------------------ consumers ------------------------------
-    const int ctid = tid;   // 0..127
+    const int ctid = tid;   // 0 .. NC-1
     T rmax = T(0);
     int slot = 0, par = 0;
-    uint32_t phase = 0;
+    uint32_t phases = 0;                       // parity of each stage's "full" barrier
+    uint32_t alive = (1u << STAGES) - 1u;      // stages whose producer has not sent its sentinel yet
+    int rot = 0;                               // tiles done: rotates which warp takes the first items of a tile
+    auto next_slot = [&]() { slot = slot == STAGES - 1 ? 0 : slot + 1; };
     for (;;) {
+        if (!((alive >> slot) & 1u)) { next_slot(); continue; }
         unsigned char* st = smem + slot * S::BYTES;
-        mbar_wait(bar_full + 8 * slot, phase);
-        const Hdr h = *reinterpret_cast<const Hdr*>(st + S::OFF_HDR);
-        if (h.quad < 0) break;
-        T* tile = reinterpret_cast<T*>(st);
-        if (h.edge) patch_boundary<T, PX, PY, XH, K>(tile, g, h.x0, h.y0, h.z0, ctid);
+        mbar_wait(bar_full + 8 * slot, (phases >> slot) & 1u);
+        phases ^= 1u << slot;
+        Hdr* hp = reinterpret_cast<Hdr*>(st + S::OFF_HDR);
+        const int quad = hp->quad;
+        if (quad < 0) {   // K = 1: this stage's producer is done; K = 2: the only producer is
+            alive &= ~(1u << slot);
+            if (K > 1 || alive == 0) break;
+            next_slot();
+            continue;
+        }
+        const int nitems = hp->nitems, edge = hp->edge;
+        TL t;
+        t.M = reinterpret_cast<T*>(st);
+        t.L = reinterpret_cast<T*>(st + S::OFF_L);
+        t.R = reinterpret_cast<T*>(st + S::OFF_R);
+        if (edge) patch_boundary<T, K, NC>(t, g, hp->x0, hp->y0, hp->z0, ctid);
         const uint16_t* items = reinterpret_cast<const uint16_t*>(st + S::OFF_ITEMS);
+
+        if (K == 2) {
+            // ---- sweep 1 on the quad's N points and on the N points of the one-cell ring around it ----
+            const unsigned char* nb = st + S::OFF_NB;
+            uint32_t* ring = reinterpret_cast<uint32_t*>(st + S::OFF_RING);
+            {   // ring list: one candidate group per consumer: face f (y-, y+, z-, z+), row r of the face, group xq
+                const int f = ctid >> 6, r = (ctid >> 3) & 7, xq = ctid & 7, j = xq >> 1;
+                int y, z, byte;
+                if (f == 0) { y = -1; z = r; byte = j * 64 + r * 8 + 7; }
+                else if (f == 1) { y = 8; z = r; byte = 256 + j * 64 + r * 8; }
+                else if (f == 2) { y = r; z = -1; byte = 512 + j * 64 + 56 + r; }
+                else { y = r; z = 8; byte = 768 + j * 64 + r; }
+                const unsigned nib = ((unsigned)nb[byte] >> ((xq & 1) * 4)) & 0xfu;
+                const unsigned vote = __ballot_sync(0xffffffffu, nib != 0);
+                int wbase = 0;
+                if (lane == 0 && vote) wbase = atomicAdd(&hp->ring_n, __popc(vote));
+                wbase = __shfl_sync(0xffffffffu, wbase, 0);
+                if (nib) ring[wbase + __popc(vote & ((1u << lane) - 1u))] = (uint32_t)(xq | ((y + 1) << 4) | ((z + 1) << 8) | (nib << 12));
+            }
+            consumer_sync<NC>();
+            const int n1 = hp->ring_n, ntot = nitems + n1;
+            constexpr int R1 = (kItemsPerQuad + 256 + NC - 1) / NC;   // rounds that cover the largest tile
+            T keep[R1][4];
+            int where[R1];
+#pragma unroll
+            for (int r = 0; r < R1; ++r) {
+                const int p = ctid + r * NC;
+                where[r] = -1;
+                if (p < ntot) {
+                    int xq, y, z;
+                    unsigned nib;
+                    if (p < nitems) {
+                        const unsigned it = items[p];
+                        nib = it >> 9; z = (it >> 6) & 7; y = (it >> 3) & 7; xq = it & 7;
+                    } else {
+                        const uint32_t e = ring[p - nitems];
+                        xq = e & 7; y = (int)((e >> 4) & 15) - 1; z = (int)((e >> 8) & 15) - 1; nib = e >> 12;
+                    }
+                    Item4<T> s;
+                    load_item<T, K>(t, xq, y, z, s);
+                    T v[4];
+                    reinit_item<T>(s, pr, v);
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) keep[r][e] = ((nib >> e) & 1u) ? v[e] : s.c[e];
+                    where[r] = TL::om(xq * 4, y, z);
+                }
+            }
+            // x ring: cells x = -1 and x = 32 of the quad's own rows, one row per thread of the first two warps
+            T xl = T(0), xr = T(0);
+            bool nl = false, nr = false;
+            int row_y = 0, row_z = 0;
+            if (ctid < 64) {
+                row_z = ctid >> 3; row_y = ctid & 7;
+                nl = (nb[1024 + row_z * 8 + row_y] >> 7) & 1;
+                nr = nb[1088 + row_z * 8 + row_y] & 1;
+                if (nl) {
+                    const int h = TL::oh(XW - 1, row_y, row_z);
+                    xl = reinit_value<T>(t.L[h], t.L[h - 1], t.M[TL::om(0, row_y, row_z)], t.L[h - XW], t.L[h + XW],
+                                         t.L[h - XW * TL::PH], t.L[h + XW * TL::PH], pr);
+                }
+                if (nr) {
+                    const int h = TL::oh(0, row_y, row_z);
+                    xr = reinit_value<T>(t.R[h], t.M[TL::om(31, row_y, row_z)], t.R[h + 1], t.R[h - XW], t.R[h + XW],
+                                         t.R[h - XW * TL::PH], t.R[h + XW * TL::PH], pr);
+                }
+            }
+            consumer_sync<NC>();   // every read of iteration k is done: write iteration k+1 in place
+#pragma unroll
+            for (int r = 0; r < R1; ++r)
+                if (where[r] >= 0) store4<T>(t.M + where[r], keep[r]);
+            if (nl) t.L[TL::oh(XW - 1, row_y, row_z)] = xl;
+            if (nr) t.R[TL::oh(0, row_y, row_z)] = xr;
+            fence_proxy_async();   // generic writes into a tile a later TMA load overwrites
+            consumer_sync<NC>();
+            if (edge) patch_boundary<T, K, NC>(t, g, hp->x0, hp->y0, hp->z0, ctid);   // edge replicate of iteration k+1
+        }
+
+        // ---- the launch's last operation on the quad's own items: results to the other global buffer ----
         const unsigned char* tm8 = st + S::OFF_TM;
         const T* Fb = reinterpret_cast<const T*>(st + S::OFF_F);
-        T* out_base = dst + h.org;
-        for (int p = ctid; p < h.nitems; p += kConsumers) {
+        T* out_base = dst + hp->org;
+        const int tvalid = hp->tvalid;
+        // A tile's items rarely fill a whole number of rounds: the warp that takes the first 32 items of every
+        // round works longest.  Rotating that role from tile to tile evens the warps out over a few tiles (the
+        // stages let them drift apart that far), so none of them ends up waiting for the slowest one.
+        const int vtid = (((warp + rot) & (NCW - 1)) << 5) | lane;
+        for (int p = vtid; p < nitems; p += NC) {
             const unsigned it = items[p];
             const unsigned nib = it >> 9;
             const int lz = (it >> 6) & 7, ly = (it >> 3) & 7, xq = it & 7;
-            const int o = ((lz + K) * PY + (ly + K)) * PX + XH + xq * 4;
             Item4<T> s;
-            load_item<T, PX, PY>(tile, o, s);
+            load_item<T, K>(t, xq, ly, lz, s);
             T v[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) v[e] = s.c[e];
             unsigned act = nib;   // cells whose value this launch changes
             if (ADV) {
-                act = h.tvalid ? ((unsigned)tm8[(xq >> 1) * 64 + lz * 8 + ly] >> ((xq & 1) * 4)) & 0xfu : 0u;
+                act = tvalid ? ((unsigned)tm8[(xq >> 1) * 64 + lz * 8 + ly] >> ((xq & 1) * 4)) & 0xfu : 0u;
                 if (act) {
                     T f[4];
                     if (sizeof(T) == 4) {
@@ -326,20 +644,21 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_src, const __grid_constant__ 
         }
         if (EMIT_T) {
             // T masks of phi^{n+1} = clamp(d) on this quad: T^{n+1} is a subset of N^n
-            consumer_sync();   // every item's bits are in
+            consumer_sync<NC>();   // every item's bits are in
             if (ctid < 32) {
                 uint64_t* w64 = reinterpret_cast<uint64_t*>(tstage + par * 64);
                 const uint64_t word = w64[ctid];
                 w64[ctid] = 0ull;   // ready for the tile after the next one (a consumer_sync lies in between)
-                a.tmask_out[(int64_t)h.quad * 32 + ctid] = word;
+                a.tmask_out[(int64_t)quad * 32 + ctid] = word;
                 const unsigned any = __ballot_sync(0xffffffffu, word != 0ull);
-                if (ctid == 0) a.qflagT_out[h.quad] = any ? 1 : 0;
+                if (ctid == 0) a.qflagT_out[quad] = any ? 1 : 0;
             }
             par ^= 1;
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_empty + 8 * slot);
-        if (++slot == STAGES) { slot = 0; phase ^= 1u; }
+        ++rot;
+        next_slot();
     }
     if (RESIDUAL) {
         // non-negative IEEE values order like their bit patterns
@@ -352,6 +671,108 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_src, const __grid_constant__ 
             bits = y > bits ? y : bits;
         }
         if (lane == 0 && bits != 0) atomicMax(a.residual, bits);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Direct variant of a K = 1 reinit sweep: no shared-memory tile.  One WARP per quad and turn; lane l evaluates
+// items l, l+32, ... of the quad's list, reading its stencil straight from the field through L1 (the rows a
+// quad touches stay resident while the warp walks the list) and writing its 16 bytes.  Latency is hidden by
+// occupancy alone.  Same arithmetic, same writes.
+// ---------------------------------------------------------------------------------------------
+#ifndef LS_DIRECT
+#define LS_DIRECT 0
+#endif
+constexpr int kDirectWarps = 8;
+template <typename T, bool CLAMP, bool RESIDUAL, bool EMIT_T>
+__global__ void __launch_bounds__(kDirectWarps * 32)
+k_band_direct(const T* __restrict__ src, T* __restrict__ dst, Geom g, StencilParams<T> pr, TileArgs a) {
+    __shared__ uint32_t s_tm[kDirectWarps][64];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int count = *a.count;
+    T rmax = T(0);
+    int base = 0;
+    for (;;) {
+        if (lane == 0) base = (int)atomicAdd(a.ticket, (unsigned)kChunk);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (base >= count) break;
+        for (int q = 0; q < kChunk && base + q < count; ++q) {
+            const QuadEntry e = a.qlist[a.reverse ? count - 1 - (base + q) : base + q];
+            const int quad = e.quad, nitems = e.nitems & 0xffff;
+            const int qx = quad % g.NQx, rest = quad / g.NQx, by = rest % g.NBy, bz = rest / g.NBy;
+            const int x0 = qx * 32, y0 = by * 8, z0 = bz * 8;
+            const bool edge = (qx == 0) | (by == 0) | (bz == 0) | (x0 + 33 > g.nx) | (y0 + 9 > g.ny) | (z0 + 9 > g.nz);
+            const uint16_t* items = a.items + (int64_t)quad * kItemsPerQuad;
+            if (EMIT_T) { s_tm[wib][lane] = 0u; s_tm[wib][lane + 32] = 0u; __syncwarp(); }
+            for (int p = lane; p < nitems; p += 32) {
+                const unsigned it = items[p];
+                const unsigned nib = it >> 9;
+                const int lz = (it >> 6) & 7, ly = (it >> 3) & 7, xq = it & 7;
+                const int x = x0 + xq * 4, y = y0 + ly, z = z0 + lz;
+                Item4<T> s;
+                auto ld4 = [&](int yy, int zz, T* o4) {
+                    const T* r = src + g.idx(x, yy, zz);
+                    if (sizeof(T) == 4) {
+                        const float4 v = __ldg(reinterpret_cast<const float4*>(r));
+                        o4[0] = (T)v.x; o4[1] = (T)v.y; o4[2] = (T)v.z; o4[3] = (T)v.w;
+                    } else {
+                        const double2 v0 = __ldg(reinterpret_cast<const double2*>(r)), v1 = __ldg(reinterpret_cast<const double2*>(r) + 1);
+                        o4[0] = (T)v0.x; o4[1] = (T)v0.y; o4[2] = (T)v1.x; o4[3] = (T)v1.y;
+                    }
+                };
+                if (!edge) {
+                    ld4(y, z, s.c); ld4(y - 1, z, s.ym); ld4(y + 1, z, s.yp); ld4(y, z - 1, s.zm); ld4(y, z + 1, s.zp);
+                    const T* r = src + g.idx(x, y, z);
+                    s.xm = __ldg(r - 1);
+                    s.xp = __ldg(r + 4);
+                } else {   // R3: edge replicate
+                    ld4(y, z, s.c); ld4(max(y - 1, 0), z, s.ym); ld4(min(y + 1, g.ny - 1), z, s.yp);
+                    ld4(y, max(z - 1, 0), s.zm); ld4(y, min(z + 1, g.nz - 1), s.zp);
+                    s.xm = __ldg(src + g.idx(max(x - 1, 0), y, z));
+                    s.xp = __ldg(src + g.idx(min(x + 4, g.nx - 1), y, z));
+                }
+                T v[4];
+                reinit_item<T>(s, pr, v);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const bool on = (nib >> k) & 1u;
+                    if (RESIDUAL && on) rmax = fmax(rmax, mag(v[k] - s.c[k]));
+                    v[k] = on ? v[k] : s.c[k];
+                    if (CLAMP) v[k] = clamp_val(v[k], pr.gamma);
+                }
+                if (EMIT_T) {
+                    unsigned tn = 0;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) tn |= (((nib >> k) & 1u) && mag(v[k]) < pr.gamma) ? (1u << k) : 0u;
+                    if (tn) atomicOr(&s_tm[wib][((xq >> 1) * 8 + lz) * 2 + (ly >> 2)], tn << ((ly & 3) * 8 + (xq & 1) * 4));
+                }
+                store4<T>(dst + g.idx(x, y, z), v);
+            }
+            if (EMIT_T) {
+                __syncwarp();
+                const uint64_t word = reinterpret_cast<const uint64_t*>(s_tm[wib])[lane];
+                a.tmask_out[(int64_t)quad * 32 + lane] = word;
+                const unsigned any = __ballot_sync(0xffffffffu, word != 0ull);
+                if (lane == 0) a.qflagT_out[quad] = any ? 1 : 0;
+                __syncwarp();
+            }
+        }
+    }
+    if (RESIDUAL) {
+        unsigned long long bits;
+        if (sizeof(T) == 4) bits = (unsigned long long)__float_as_uint((float)rmax);
+        else bits = (unsigned long long)__double_as_longlong((double)rmax);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const unsigned long long y = __shfl_xor_sync(0xffffffffu, bits, o);
+            bits = y > bits ? y : bits;
+        }
+        if (lane == 0 && bits != 0) atomicMax(a.residual, bits);
+    }
+    // self-resetting scheduler: the last warp to finish fetching zeroes the counters for the next launch
+    if (lane == 0) {
+        __threadfence();
+        if (atomicAdd(a.ticket + 1, 1u) == gridDim.x * kDirectWarps - 1) { a.ticket[0] = 0u; a.ticket[1] = 0u; }
     }
 }
 
@@ -392,27 +813,31 @@ bool make_map(CUtensorMap* m, const void* field, const Geom& g, int bx, int by, 
 
 // Persistent grid of a band kernel: the largest shared-memory carve-out, then as many CTAs as fit on an SM.
 template <typename Kn>
-int persistent_grid(Kn kernel, size_t dyn_smem) {
+int persistent_grid(Kn kernel, int threads, size_t dyn_smem) {
     cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_smem);
     cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kThreads, dyn_smem) != cudaSuccess || per_sm < 1) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, dyn_smem) != cudaSuccess || per_sm < 1) {
         cudaGetLastError();
         per_sm = 1;
     }
     return sm_count() * per_sm;
 }
 
-template <typename T, bool ADV, int SWEEPS, bool CLAMP, bool RESIDUAL, bool EMIT_T>
-void launch_variant(const CUtensorMap& tm_src, const CUtensorMap& tm_F, T* dst, const Geom& g, const StencilParams<T>& pa,
-                    const StencilParams<T>& pr, const TileArgs& a, cudaStream_t s) {
-    constexpr int K = (ADV ? 1 : 0) + SWEEPS;
-    constexpr int STAGES = (ADV || sizeof(T) == 8) ? 2 : 3;
+struct Maps { CUtensorMap M, H, F; };
+
+template <typename T, bool ADV, int K, bool CLAMP, bool RESIDUAL, bool EMIT_T>
+void launch_variant(const Maps& m, T* dst, const Geom& g, const StencilParams<T>& pa, const StencilParams<T>& pr,
+                    const TileArgs& a, cudaStream_t s) {
+    constexpr int NCW = K > 1 ? 8 : 4;
+    constexpr int STAGES = (K > 1 || ADV || sizeof(T) == 8) ? 2 : 3;
+    constexpr int NPW = K > 1 ? 1 : STAGES;   // K = 1: one gather warp per stage; K = 2: one lane issuing TMA boxes
     using S = Stage<T, K, ADV>;
     const size_t shm = (size_t)STAGES * S::BYTES + 512 + 16 * STAGES;
-    auto kern = k_band_tile<T, ADV, SWEEPS, CLAMP, RESIDUAL, EMIT_T, STAGES>;
-    static const int grid = persistent_grid(kern, shm);
-    kern<<<grid, kThreads, shm, s>>>(tm_src, tm_F, dst, g, pa, pr, a);
+    auto kern = k_band_tile<T, ADV, K, CLAMP, RESIDUAL, EMIT_T, STAGES, NCW, NPW>;
+    // (the grid is sized once per process for the device current at the first launch: every B200 is alike)
+    static const int grid = persistent_grid(kern, (NCW + NPW) * 32, shm);
+    kern<<<grid, (NCW + NPW) * 32, shm, s>>>(m.M, m.H, m.F, dst, g, pa, pr, a);
 }
 
 }  // namespace
@@ -429,33 +854,52 @@ template <typename T>
 bool launch_band_tile(const T* src, const T* F, T* dst, const Geom& g, const StencilParams<T>& p, const BandBuffers& bb,
                       const BandOp& op, cudaStream_t s, int64_t* launches) {
     const int K = (op.advance ? 1 : 0) + op.sweeps;
-    if (K != 1) return false;
-    constexpr int XH = XHalo<T>::XH;
-    CUtensorMap tm_src, tm_F;
-    if (!make_map<T>(&tm_src, src, g, 32 + 2 * XH, 8 + 2 * K, 8 + 2 * K)) return false;
+    if (K < 1 || K > 2 || (op.advance && K != 1)) return false;
+    constexpr int XW = 16 / (int)sizeof(T);
+    Maps m;
+    if (!make_map<T>(&m.M, src, g, 32, 8 + 2 * K, 8 + 2 * K)) return false;
+    if (!make_map<T>(&m.H, src, g, XW, 6 + 2 * K, 6 + 2 * K)) return false;
     if (op.advance) {
-        if (!make_map<T>(&tm_F, F, g, 32, 8, 8)) return false;
+        if (!make_map<T>(&m.F, F, g, 32, 8, 8)) return false;
     } else {
-        tm_F = tm_src;
+        m.F = m.M;
     }
     TileArgs a;
     a.qlist = bb.qlist[op.list];
     a.count = &bb.counts->nQ[op.list];
     a.items = bb.items[op.list];
+    a.qneed = bb.qneed[op.list];
+    a.nmask = bb.nmask;
+    a.zero_page = bb.zero_page;
     a.tmask_in = bb.tmask[bb.tb];
     a.qflagT_in = bb.qflagT[bb.tb];
     a.tgate = op.tgate;
     a.tmask_out = bb.tmask[bb.tb ^ 1];
     a.qflagT_out = bb.qflagT[bb.tb ^ 1];
     a.residual = op.residual;
+    a.src = src;
+    a.F = F;
     a.ticket = bb.counts->ticket;
     a.reverse = op.reverse ? 1 : 0;
-    if (op.advance) launch_variant<T, true, 0, false, false, false>(tm_src, tm_F, dst, g, p, p, a, s);
-    else if (op.emit_T) launch_variant<T, false, 1, true, false, true>(tm_src, tm_F, dst, g, p, p, a, s);
-    else if (op.residual && op.clamp) launch_variant<T, false, 1, true, true, false>(tm_src, tm_F, dst, g, p, p, a, s);
-    else if (op.residual) launch_variant<T, false, 1, false, true, false>(tm_src, tm_F, dst, g, p, p, a, s);
-    else if (op.clamp) launch_variant<T, false, 1, true, false, false>(tm_src, tm_F, dst, g, p, p, a, s);
-    else launch_variant<T, false, 1, false, false, false>(tm_src, tm_F, dst, g, p, p, a, s);
+#define LS_VARIANTS(KK)                                                                                      \
+    do {                                                                                                     \
+        if (op.emit_T) launch_variant<T, false, KK, true, false, true>(m, dst, g, p, p, a, s);               \
+        else if (op.residual && op.clamp) launch_variant<T, false, KK, true, true, false>(m, dst, g, p, p, a, s);  \
+        else if (op.residual) launch_variant<T, false, KK, false, true, false>(m, dst, g, p, p, a, s);       \
+        else if (op.clamp) launch_variant<T, false, KK, true, false, false>(m, dst, g, p, p, a, s);          \
+        else launch_variant<T, false, KK, false, false, false>(m, dst, g, p, p, a, s);                       \
+    } while (0)
+    if (LS_DIRECT && !op.advance && K == 1) {
+        static const int dgrid = [] { int n = 0; cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_band_direct<T, false, false, false>, kDirectWarps * 32, 0); return sm_count() * (n > 0 ? n : 1); }();
+        if (op.emit_T) k_band_direct<T, true, false, true><<<dgrid, kDirectWarps * 32, 0, s>>>(src, dst, g, p, a);
+        else if (op.residual && op.clamp) k_band_direct<T, true, true, false><<<dgrid, kDirectWarps * 32, 0, s>>>(src, dst, g, p, a);
+        else if (op.residual) k_band_direct<T, false, true, false><<<dgrid, kDirectWarps * 32, 0, s>>>(src, dst, g, p, a);
+        else if (op.clamp) k_band_direct<T, true, false, false><<<dgrid, kDirectWarps * 32, 0, s>>>(src, dst, g, p, a);
+        else k_band_direct<T, false, false, false><<<dgrid, kDirectWarps * 32, 0, s>>>(src, dst, g, p, a);
+    } else if (op.advance) launch_variant<T, true, 1, false, false, false>(m, dst, g, p, p, a, s);
+    else if (K == 2) LS_VARIANTS(2);
+    else LS_VARIANTS(1);
+#undef LS_VARIANTS
     if (launches) *launches += 1;
     return true;
 }

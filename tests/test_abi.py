@@ -43,7 +43,7 @@ def test_status_strings(lib):
 def test_params_struct_layout():
     assert C.sizeof(ls.ls_params) == 56
     assert ls.ls_params.iters.offset == 40 and ls.ls_params.rebuild.offset == 44
-    assert ls.ls_params.chained.offset == 48 and ls.ls_params.reserved.offset == 52
+    assert ls.ls_params.chained.offset == 48 and ls.ls_params.fuse.offset == 52
 
 
 def test_bad_arguments_rejected_before_cuda(lib):
@@ -90,7 +90,8 @@ def test_packed_fp32_arithmetic_is_not_contracted():
       reinit sweep, per pair: 6 differences + 5 sums + den^2 + 2 sqrt seeds + (g - 1) + (c - dtau U) = 16 FADD2;
         6 scalings + 2x2 sqrt + U = 11 FMUL2; 6 squares + 2 (den^2) + 2x2 sqrt + 5 divide + dtau U = 18 FFMA2
       Advance, per pair: 16 FADD2, 13 FMUL2, 10 FFMA2
-    and two pairs per item.  A different count means the toolchain fused (or split) something: fail here, on
+    and two pairs per item; the two-sweep kernels (temporal blocking) hold four copies of the sweep (three
+    unrolled rounds of sweep 1 and sweep 2).  A different count means the toolchain fused (or split) something: fail here, on
     the CPU.  (The scalar slow path of the same kernels uses FADD / FMUL / FFMA, which are not counted.)"""
     import re
     import shutil
@@ -116,13 +117,17 @@ def test_packed_fp32_arithmetic_is_not_contracted():
                 counts[fn][op] += 1
         if "UTMALDG" in line or "UBLKCP" in line:
             tma_ops[fn] = tma_ops.get(fn, 0) + 1
-    # mangled: k_band_tile<float, ADV, SWEEPS, ...> -> "k_band_tileIfLb0ELi1E..." (reinit) / "k_band_tileIfLb1ELi0E..." (advance)
+    # mangled: k_band_tile<float, ADV, K, ...> -> "k_band_tileIfLb0ELi1E..." (one sweep), "...IfLb0ELi2E..." (two
+    # sweeps), "...IfLb1ELi1E..." (advance)
     reinit_f32 = [f for f in counts if "k_band_tileIfLb0ELi1E" in f]
-    advance_f32 = [f for f in counts if "k_band_tileIfLb1ELi0E" in f]
-    assert len(reinit_f32) == 5 and len(advance_f32) == 1, (reinit_f32, advance_f32)
+    reinit2_f32 = [f for f in counts if "k_band_tileIfLb0ELi2E" in f]
+    advance_f32 = [f for f in counts if "k_band_tileIfLb1ELi1E" in f]
+    assert len(reinit_f32) == 5 and len(reinit2_f32) == 5 and len(advance_f32) == 1, (reinit_f32, reinit2_f32, advance_f32)
     for f in reinit_f32:
         assert counts[f] == {"FFMA2": 36, "FMUL2": 22, "FADD2": 32}, (f, counts[f])
+    for f in reinit2_f32:
+        assert counts[f] == {"FFMA2": 144, "FMUL2": 88, "FADD2": 128}, (f, counts[f])
     assert counts[advance_f32[0]] == {"FFMA2": 20, "FMUL2": 26, "FADD2": 32}, counts[advance_f32[0]]
     # and the band kernels really are TMA kernels (cp.async.bulk.tensor -> UTMALDG, cp.async.bulk -> UBLKCP)
-    for f in reinit_f32 + advance_f32:
+    for f in reinit_f32 + reinit2_f32 + advance_f32:
         assert tma_ops.get(f, 0) >= 2, f

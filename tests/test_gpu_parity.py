@@ -240,16 +240,19 @@ def test_step_chained_falls_back_when_phi_differs():
         assert np.array_equal(b.cpu().numpy(), want4)
 
 
-def test_profile_counts_launches():
+@pytest.mark.parametrize("fuse,reinit_launches", [(1, 15), (2, 9), (0, 9)])
+def test_profile_counts_launches(fuse, reinit_launches):
+    """Per-kernel event brackets: 3 steps of 5 sweeps are 15 launches with one sweep per launch and 9 with two
+    (2 + 2 + 1, an odd number of launches so that the last one lands in phi)."""
     w = inputs.config(1, n=32)
-    p = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, ls.LS_REBUILD_INCREMENTAL)
+    p = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, ls.LS_REBUILD_INCREMENTAL, 0, fuse)
     with Ctx(w.shape, w.dtype) as ctx:
         d_phi, d_F = to_dev(w.phi), to_dev(w.F)
         ls.ls_profile_enable(ctx, True)
         ls.ls_step(ctx, d_phi, d_F, p, 3)
         got = {name: ls.ls_profile_read(ctx, k) for k, name in enumerate(ls.KERNEL_KINDS)}
         ls.ls_profile_enable(ctx, False)
-        assert got["reinit"][1] == 15 and got["advance"][1] == 3 and got["band"][1] == 3
+        assert got["reinit"][1] == reinit_launches and got["advance"][1] == 3 and got["band"][1] == 3
         assert got["classify"][1] == 1 and got["copy"][1] == 1 and got["clamp"][1] == 1
         assert all(ms > 0 for ms, n in got.values() if n)
         ls.ls_profile_reset(ctx)
