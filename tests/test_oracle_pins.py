@@ -428,3 +428,94 @@ def test_reinit_tol_stops_on_the_residual_rule():
     assert np.abs(np.abs(gz) - 1).max() < 1e-6               # a tilted plane relaxes to slope 1
     d2, k2, r2, conv2 = orc.reinit_tol(phi, 0.3 * dx, dx, 8 * dx, 1e-30, 7, check_every=1)
     assert not conv2 and k2 == 7
+
+
+# ---------------------------------------------------------------- outputs the pins above do not reach
+def _perturbed_sphere(n, dtype, amp=0.35):
+    dx = 1.0 / n
+    x = (np.arange(n) + 0.5) * dx
+    X, Y, Z = x[None, None, :], x[None, :, None], x[:, None, None]
+    sdf = np.sqrt((X - 0.5) ** 2 + (Y - 0.5) ** 2 + (Z - 0.5) ** 2) - 0.3
+    return (sdf * (1.0 + amp * np.sin(9 * X + 1) * np.cos(7 * Y) * np.sin(8 * Z + 2))).astype(dtype), dx
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_reinit_iter_residual_is_max_abs_change_over_N(dtype):
+    """Stopping rule of eq. 12 (R13): r = max_{x in N} |d^{k+1} - d^k|, an ABSOLUTE value taken
+    over N only.  Two fields: one whose largest change is a DECREASE (slope 2, d > 0: eq. 12 lowers d), so a
+    signed maximum would come out smaller or negative; one where a big change lies outside N and must not count."""
+    n = 9
+    x = np.arange(n, dtype=np.float64) - 4
+    d = np.broadcast_to((3 * x + 13)[None, None, :], (n, n, n)).astype(dtype).copy()   # d > 0 everywhere, |grad| = 3
+    Nm = np.ones(d.shape, np.uint8)
+    out, r = orc.reinit_iter(d, Nm, 0.25, 1.0)
+    diff = out.astype(np.float64) - d.astype(np.float64)
+    # interior points move DOWN by ~0.5 (|grad| = 3 > 1); only the x = 0 face (edge replicate: upwind |grad| = 0)
+    # moves up, by < 0.25: a signed maximum would report that face instead
+    assert diff.min() < -0.45 and 0.0 < diff.max() < 0.26
+    assert r == np.abs(diff).max() and r > 0.45
+    # restricted to N: the steep half is outside N
+    d2 = d.copy()
+    d2[:, :, :4] = d2[:, :, 3:4] + (x[:4] - x[3])[None, None, :].astype(dtype)   # |grad| = 1 for x <= 3: nearly still
+    Nm2 = np.zeros(d.shape, np.uint8)
+    Nm2[:, :, :3] = 1
+    out2, r2 = orc.reinit_iter(d2, Nm2, 0.25, 1.0)
+    diff2 = np.abs(out2.astype(np.float64) - d2.astype(np.float64))
+    assert np.array_equal(out2[Nm2 == 0], d2[Nm2 == 0])
+    assert r2 == diff2[Nm2 == 1].max()
+    full2, rfull = orc.reinit_iter(d2, Nm, 0.25, 1.0)
+    assert rfull > r2                                          # the steep part would have dominated
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_reinit_tol_iterates_on_N_and_clamps_everywhere(dtype):
+    """Step 3 runs "on the tube N" (eq. 11), not on T, and eq. 10 (R14) is
+    applied at every point afterwards.  Built from the single-iteration function (pinned above) and numpy:
+    k x reinit_iter on the N mask of numpy's own dilation, then numpy's clip."""
+    n = 24
+    phi, dx = _perturbed_sphere(n, dtype)
+    gamma = 4 * dx
+    phi[2, 3, 4] = dtype(11 * dx)                               # far outside N and beyond +-gamma: only eq. 10 moves them
+    phi[20, 20, 3] = dtype(-9 * dx)
+    Tm = (np.abs(phi) < dtype(gamma))
+    Nm = np_dilate6(Tm).astype(np.uint8)
+    k = 7
+    d = phi.copy()
+    for _ in range(k):
+        d, r_last = orc.reinit_iter(d, Nm, 0.3 * dx, dx)
+    moved_rim = (d != phi) & (Nm == 1) & ~Tm
+    assert moved_rim.sum() > 50                                 # points of N \ T do move: T-only iteration differs
+    on_T = phi.copy()
+    for _ in range(k):
+        on_T, _ = orc.reinit_iter(on_T, Tm.astype(np.uint8), 0.3 * dx, dx)
+    want = np.clip(d, dtype(-gamma), dtype(gamma))
+    assert not np.array_equal(np.clip(on_T, dtype(-gamma), dtype(gamma)), want)
+    assert np.abs(d).max() > dtype(gamma)                       # and the clamp has something to do
+    got, kk, r, conv = orc.reinit_tol(phi, 0.3 * dx, dx, gamma, 1e-30, k, check_every=1)
+    assert kk == k and not conv and r == r_last
+    assert np.array_equal(got, want)
+    assert got[2, 3, 4] == dtype(gamma) and got[20, 20, 3] == dtype(-gamma)
+    # a check that is not yet due must not stop the iteration: tol is met from the start, check_every = 5
+    flat_ok, k5, _, conv5 = orc.reinit_tol(phi, 0.3 * dx, dx, gamma, 1e30, 12, check_every=5)
+    assert conv5 and k5 == 5
+
+
+@pytest.mark.parametrize("use_lists", [False, True])
+def test_step_update_count_is_T_plus_iters_times_N(use_lists):
+    """The metric's numerator: sum over steps of |T_s| + iters * |N_s|, with T_s, N_s the
+    tubes of phi^s (Step 1) — recomputed here with numpy along the oracle's own trajectory."""
+    n = 24
+    w = inputs.config(1, n=n)
+    F = rnd((n, n, n), 21, np.float32)
+    iters = 3
+    phi = w.phi
+    total = 0
+    for s in range(4):
+        Tm = np.abs(phi) < np.float32(w.gamma)
+        Nm = np_dilate6(Tm)
+        assert Nm.sum() > Tm.sum() > 0
+        total += int(Tm.sum()) + iters * int(Nm.sum())
+        phi, u1 = orc.step(phi, F, w.dx, w.dt, w.dtau, w.beta, w.gamma, iters, 1, use_lists=use_lists)
+        assert u1 == int(Tm.sum()) + iters * int(Nm.sum())
+    _, u4 = orc.step(w.phi, F, w.dx, w.dt, w.dtau, w.beta, w.gamma, iters, 4, use_lists=use_lists)
+    assert u4 == total
