@@ -58,7 +58,7 @@ def parse_args():
     ap.add_argument("--n", type=int, default=None, help="grid edge override (smoke runs of the bench itself)")
     ap.add_argument("--rebuild", default="incremental", choices=["incremental", "full"])
     ap.add_argument("--fuse", type=int, default=0, choices=[0, 1, 2],
-                    help="reinit sweeps per launch: 0 = library default (2), 1 = no temporal blocking, 2")
+                    help="reinit sweeps per launch: 0 = library default (1), 1 = one sweep per launch, 2 = temporal blocking")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()

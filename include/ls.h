@@ -71,11 +71,13 @@ typedef struct {
                         field and (LS_REBUILD_INCREMENTAL) the T masks it emitted from phi^n, so the call
                         does no whole-grid work at all: no resync copy, no scan, no global clamp.  If the
                         ctx cannot verify pointer / gamma / state it silently runs the unchained path. */
-    int32_t fuse;     /* reinit sweeps per kernel launch: 0 = library default (2), 1 = one launch per sweep, 2 = two
+    int32_t fuse;     /* reinit sweeps per kernel launch: 0 = library default (1), 1 = one launch per sweep, 2 = two
                          sweeps per launch where the grid allows it (temporal blocking of eq. 12's iterations in
                          shared memory: the tile is loaded once, sweep k is evaluated on the tile's N points and on
                          the one-cell ring around it, sweep k+1 on the tile's own points).  The results do not
-                         depend on it: Jacobi order is kept exactly. */
+                         depend on it: Jacobi order is kept exactly.  One sweep per launch is the default because it
+                         is the faster one on B200 (the sweeps are bound by instruction issue, not by memory traffic,
+                         and the ring costs extra evaluations: DESIGN.md section 6). */
 } ls_params;
 
 /* Kernel classes of the per-kernel device timing (ls_profile_*). */

@@ -228,7 +228,7 @@ ls_status step_impl(ls_ctx* c, T* phi, const T* F, const ls_params* p, int n_ste
         // Step 3: `iters` sweeps in launches of 2 (temporal blocking, tile path only) or 1.  The number of
         // launches should be odd so that the last one lands in phi; if it cannot be (iters == 0, or an even
         // count on the scalar path), the band copy below moves the result.
-        const bool can_fuse = p->fuse != 1 && ls::tile_usable<T>(c->g, phi, S, (const void*)nullptr);
+        const bool can_fuse = p->fuse == 2 && ls::tile_usable<T>(c->g, phi, S, (const void*)nullptr);
         int pairs = can_fuse ? p->iters / 2 : 0, singles = p->iters - 2 * pairs;
         if (pairs > 0 && ((pairs + singles) & 1) == 0) { pairs -= 1; singles += 2; }
         for (int l = 0; l < pairs + singles; ++l) {

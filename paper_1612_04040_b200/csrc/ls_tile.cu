@@ -245,15 +245,16 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_M, const __grid_constant__ CU
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t smem_base = smem_u32(smem);
-    // after the stages: T staging of EMIT_T (2 x 256 B), then the mbarriers (full[STAGES], empty[STAGES])
-    uint32_t* tstage = reinterpret_cast<uint32_t*>(smem + STAGES * S::BYTES);
-    const uint32_t bar_full = smem_base + STAGES * S::BYTES + 512, bar_empty = bar_full + 8 * STAGES;
+    // after the stages: T staging of EMIT_T (2 x 512 B: one byte per item position), then the mbarriers
+    // (full[STAGES], empty[STAGES])
+    unsigned char* tstage = smem + STAGES * S::BYTES;
+    const uint32_t bar_full = smem_base + STAGES * S::BYTES + 1024, bar_empty = bar_full + 8 * STAGES;
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < STAGES; ++s) { mbar_init(bar_full + 8 * s, K == 1 ? 33 : 1); mbar_init(bar_empty + 8 * s, NCW); }
         fence_barrier_init();
     }
-    if (EMIT_T && tid < 128) tstage[tid] = 0u;
+    if (EMIT_T && tid < 64) reinterpret_cast<uint4*>(tstage)[tid] = make_uint4(0u, 0u, 0u, 0u);
     // K = 1 fetches only the chunks its items read; the rest of a stage keeps what earlier tiles left there, which
     // only feeds results that are thrown away (cells of an item outside N).  Start from zeros, not from whatever
     // bit patterns the last kernel left in shared memory (a NaN would send a lane down the scalar slow path).
@@ -634,11 +635,11 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_M, const __grid_constant__ CU
                 v[e] = on ? v[e] : s.c[e];
                 if (CLAMP) v[e] = clamp_val(v[e], pr.gamma);
             }
-            if (EMIT_T) {
+            if (EMIT_T) {   // T of phi^{n+1} = clamp(d) at the item's N cells: one staging byte per item, no atomics
                 unsigned tn = 0;
 #pragma unroll
                 for (int e = 0; e < 4; ++e) tn |= (((nib >> e) & 1u) && mag(v[e]) < pr.gamma) ? (1u << e) : 0u;
-                if (tn) atomicOr(tstage + par * 64 + ((xq >> 1) * 8 + lz) * 2 + (ly >> 2), tn << ((ly & 3) * 8 + (xq & 1) * 4));
+                tstage[par * 512 + (it & 511u)] = (unsigned char)tn;
             }
             store4<T>(out_base + (int64_t)(lz * g.ny + ly) * g.nx + xq * 4, v);
         }
@@ -646,9 +647,18 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_M, const __grid_constant__ CU
             // T masks of phi^{n+1} = clamp(d) on this quad: T^{n+1} is a subset of N^n
             consumer_sync<NC>();   // every item's bits are in
             if (ctid < 32) {
-                uint64_t* w64 = reinterpret_cast<uint64_t*>(tstage + par * 64);
-                const uint64_t word = w64[ctid];
-                w64[ctid] = 0ull;   // ready for the tile after the next one (a consumer_sync lies in between)
+                // lane (j, lz) packs the staging bytes of its brick layer (two item nibbles per mask byte) into word lz
+                // of brick j, then clears them for the tile after the next one (a consumer_sync lies in between)
+                unsigned char* ts = tstage + par * 512;
+                const int j = ctid >> 3, lz = ctid & 7;
+                uint64_t word = 0ull;
+#pragma unroll
+                for (int ly = 0; ly < 8; ++ly) {
+                    const unsigned two = *reinterpret_cast<const unsigned short*>(ts + lz * 64 + ly * 8 + 2 * j);
+                    word |= (uint64_t)((two & 0xfu) | ((two >> 4) & 0xf0u)) << (8 * ly);
+                }
+                __syncwarp();
+                reinterpret_cast<uint4*>(ts)[ctid] = make_uint4(0u, 0u, 0u, 0u);
                 a.tmask_out[(int64_t)quad * 32 + ctid] = word;
                 const unsigned any = __ballot_sync(0xffffffffu, word != 0ull);
                 if (ctid == 0) a.qflagT_out[quad] = any ? 1 : 0;
@@ -833,7 +843,7 @@ void launch_variant(const Maps& m, T* dst, const Geom& g, const StencilParams<T>
     constexpr int STAGES = (K > 1 || ADV || sizeof(T) == 8) ? 2 : 3;
     constexpr int NPW = K > 1 ? 1 : STAGES;   // K = 1: one gather warp per stage; K = 2: one lane issuing TMA boxes
     using S = Stage<T, K, ADV>;
-    const size_t shm = (size_t)STAGES * S::BYTES + 512 + 16 * STAGES;
+    const size_t shm = (size_t)STAGES * S::BYTES + 1024 + 16 * STAGES;
     auto kern = k_band_tile<T, ADV, K, CLAMP, RESIDUAL, EMIT_T, STAGES, NCW, NPW>;
     // (the grid is sized once per process for the device current at the first launch: every B200 is alike)
     static const int grid = persistent_grid(kern, (NCW + NPW) * 32, shm);

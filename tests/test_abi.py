@@ -102,7 +102,7 @@ def test_packed_fp32_arithmetic_is_not_contracted():
     from paper_1612_04040_b200 import build as ls_build
     so = ls_build.build()
     sass = subprocess.run([cuobjdump, "-sass", str(so)], capture_output=True, text=True, check=True).stdout
-    counts, tma_ops = {}, {}
+    counts, tma_ops, ldgsts = {}, {}, {}
     fn = None
     for line in sass.splitlines():
         m = re.search(r"Function : (\S+)", line)
@@ -117,6 +117,8 @@ def test_packed_fp32_arithmetic_is_not_contracted():
                 counts[fn][op] += 1
         if "UTMALDG" in line or "UBLKCP" in line:
             tma_ops[fn] = tma_ops.get(fn, 0) + 1
+        if "LDGSTS" in line:
+            ldgsts[fn] = ldgsts.get(fn, 0) + 1
     # mangled: k_band_tile<float, ADV, K, ...> -> "k_band_tileIfLb0ELi1E..." (one sweep), "...IfLb0ELi2E..." (two
     # sweeps), "...IfLb1ELi1E..." (advance)
     reinit_f32 = [f for f in counts if "k_band_tileIfLb0ELi1E" in f]
@@ -128,6 +130,10 @@ def test_packed_fp32_arithmetic_is_not_contracted():
     for f in reinit2_f32:
         assert counts[f] == {"FFMA2": 144, "FMUL2": 88, "FADD2": 128}, (f, counts[f])
     assert counts[advance_f32[0]] == {"FFMA2": 20, "FMUL2": 26, "FADD2": 32}, counts[advance_f32[0]]
-    # and the band kernels really are TMA kernels (cp.async.bulk.tensor -> UTMALDG, cp.async.bulk -> UBLKCP)
-    for f in reinit_f32 + reinit2_f32 + advance_f32:
+    # and the band kernels really use the asynchronous copy paths: the two-sweep kernels take whole boxes by TMA
+    # (cp.async.bulk.tensor -> UTMALDG); the one-sweep kernels gather the sectors they need with cp.async (LDGSTS) and
+    # take the item list by cp.async.bulk (UBLKCP)
+    for f in reinit2_f32:
         assert tma_ops.get(f, 0) >= 2, f
+    for f in reinit_f32 + advance_f32:
+        assert tma_ops.get(f, 0) >= 1 and ldgsts.get(f, 0) >= 4, f

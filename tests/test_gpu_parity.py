@@ -240,7 +240,7 @@ def test_step_chained_falls_back_when_phi_differs():
         assert np.array_equal(b.cpu().numpy(), want4)
 
 
-@pytest.mark.parametrize("fuse,reinit_launches", [(1, 15), (2, 9), (0, 9)])
+@pytest.mark.parametrize("fuse,reinit_launches", [(1, 15), (2, 9), (0, 15)])
 def test_profile_counts_launches(fuse, reinit_launches):
     """Per-kernel event brackets: 3 steps of 5 sweeps are 15 launches with one sweep per launch and 9 with two
     (2 + 2 + 1, an odd number of launches so that the last one lands in phi)."""
@@ -257,6 +257,31 @@ def test_profile_counts_launches(fuse, reinit_launches):
         assert all(ms > 0 for ms, n in got.values() if n)
         ls.ls_profile_reset(ctx)
         assert ls.ls_profile_read(ctx, ls.LS_K_REINIT) == (0.0, 0)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("shape", [(20, 13, 40), (33, 17, 64), (24, 40, 56), (64, 64, 64)])
+def test_fused_sweeps_equal_single_sweeps(shape, dtype):
+    """Temporal blocking (ls_params.fuse = 2: two eq. 12 iterations per staged tile) keeps Jacobi order
+    exactly: free-running steps with fused sweeps equal the same steps with one launch per sweep AND the oracle, bit
+    for bit, on ragged shapes whose band touches the domain boundary; iters = 5 (2 + 2 + 1) and 4 (2 + 1 + 1)."""
+    dx = 1.0 / 32
+    phi, F = _random_band_field(shape, dtype, 71, dx)
+    F = (0.6 * F).astype(dtype)
+    gamma, beta, dt, dtau = 4 * dx, 2 * dx, 0.4 * dx, 0.5 * dx
+    for iters in (5, 4):
+        want, _ = orc.step(phi, F, dx, dt, dtau, beta, gamma, iters, 3)
+        got = {}
+        for fuse in (1, 2):
+            with Ctx(shape, dtype) as ctx:
+                d_phi, d_F = to_dev(phi), to_dev(F)
+                ls.ls_step(ctx, d_phi, d_F, ls.make_params(dx, dt, dtau, beta, gamma, iters, ls.LS_REBUILD_INCREMENTAL, 0, fuse), 3)
+                got[fuse] = d_phi.cpu().numpy()
+                launches = ls.ls_stats(ctx)[2]
+            got[(fuse, "launches")] = launches
+        assert got[(2, "launches")] < got[(1, "launches")]          # the fused path really ran
+        assert np.array_equal(got[1], got[2])
+        assert np.array_equal(got[2], want)
 
 
 def test_step_ragged_fp64():
