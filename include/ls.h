@@ -156,7 +156,9 @@ ls_status ls_reinit_tol(ls_ctx* ctx, void* d, const void* phi_bar, double dtau, 
 ls_status ls_step(ls_ctx* ctx, void* phi, const void* F, const ls_params* p, int32_t n_steps);
 
 /* Same as ls_step with HOST buffers (pageable or pinned): copies phi and F to ctx-owned device
- * fields, runs n_steps, copies phi back, and synchronises.  The end-to-end entry point. */
+ * fields, runs n_steps, copies phi back, and synchronises.  The end-to-end entry point.
+ * F is static (R17): F_host = NULL reuses the F that the last call with a non-NULL F_host left on the
+ * device (LS_ERR_STATE if there was none), which saves a third of the transfer. */
 ls_status ls_step_host(ls_ctx* ctx, void* phi_host, const void* F_host, const ls_params* p, int32_t n_steps);
 
 /* m-step batching with snapshot return (the paper keeps m results on the device and
@@ -167,7 +169,8 @@ ls_status ls_step_host(ls_ctx* ctx, void* phi_host, const void* F_host, const ls
  * Snapshot k is copied device-to-device into one of two ctx-owned slots on the ctx stream, and from the slot
  * to the host on a second, ctx-owned stream while the following steps compute (events order the two
  * streams both ways).  `phi` is updated in place as by ls_step.  Synchronises both streams before it
- * returns.  HOST out-pointer n_written (may be NULL) = number of snapshots written.
+ * returns, also when a step or a copy fails (then the first error is returned).  HOST out-pointer n_written (may be
+ * NULL) = number of snapshots written.
  * p->chained is honoured for the first step; the remaining steps are chained internally. */
 ls_status ls_step_snapshots(ls_ctx* ctx, void* phi, const void* F, const ls_params* p, int32_t n_steps,
                             int32_t every, void* host_out, int32_t* n_written);

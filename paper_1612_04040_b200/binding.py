@@ -172,7 +172,9 @@ def ls_step(ctx: int, phi, F, p: ls_params, n_steps: int) -> None:
 
 
 def ls_step_host(ctx: int, phi_host, F_host, p: ls_params, n_steps: int) -> None:
-    _ck(lib().ls_step_host(_P(ctx), _P(_host(phi_host)), _P(_host(F_host)), C.byref(p), n_steps), "ls_step_host")
+    """F_host=None: reuse the F the last call with an F_host left on the device."""
+    f = _P(None) if F_host is None else _P(_host(F_host))
+    _ck(lib().ls_step_host(_P(ctx), _P(_host(phi_host)), f, C.byref(p), n_steps), "ls_step_host")
 
 
 def ls_stats(ctx: int):

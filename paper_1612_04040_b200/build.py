@@ -32,6 +32,17 @@ def nvcc_path() -> str:
     raise RuntimeError("nvcc not found: libls.so cannot be built (there is no CPU fallback)")
 
 
+def source_sha() -> str:
+    """Hash of the kernel sources (csrc/ and include/ls.h): ties an ncu capture summary to the code it measured."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(CSRC.iterdir()) + [PKG.parent / "include" / "ls.h"]:
+        if f.suffix in (".cu", ".cuh", ".h"):
+            h.update(f.name.encode())
+            h.update(f.read_bytes())
+    return h.hexdigest()[:16]
+
+
 def needs_build() -> bool:
     if not SO.exists():
         return True

@@ -21,6 +21,7 @@ struct ls_ctx {
     void* scratch;        // one field, second Jacobi buffer (lazy)
     void* dev_phi;        // ls_step_host staging (lazy)
     void* dev_F;
+    bool dev_F_valid;     // dev_F holds the F of the last ls_step_host call that passed one
     void* snap[2];        // ls_step_snapshots: device snapshot slots (lazy)
     cudaStream_t copy_stream;   // ... and the stream / events of the device-to-host copies (lazy)
     cudaEvent_t snap_ready[2], snap_free[2];
@@ -559,13 +560,19 @@ ls_status ls_step(ls_ctx* c, void* phi, const void* F, const ls_params* p, int32
 }
 
 ls_status ls_step_host(ls_ctx* c, void* phi_host, const void* F_host, const ls_params* p, int32_t n_steps) {
-    ls_status st = check_step_args(c, phi_host, F_host, p, n_steps);
+    // F_host == NULL: reuse the F uploaded by the last call that passed one (R17: F is static)
+    if (!F_host && c && !c->dev_F_valid) return LS_ERR_STATE;
+    ls_status st = check_step_args(c, phi_host, F_host ? F_host : (const void*)phi_host, p, n_steps);
     if (st != LS_OK) return st;
     if ((st = ensure_field(c, &c->dev_phi)) != LS_OK) return st;
     if ((st = ensure_field(c, &c->dev_F)) != LS_OK) return st;
     const size_t bytes = (size_t)c->n * c->elem;
     LS_CK(cudaMemcpyAsync(c->dev_phi, phi_host, bytes, cudaMemcpyHostToDevice, c->stream));
-    LS_CK(cudaMemcpyAsync(c->dev_F, F_host, bytes, cudaMemcpyHostToDevice, c->stream));
+    if (F_host) {
+        c->dev_F_valid = false;
+        LS_CK(cudaMemcpyAsync(c->dev_F, F_host, bytes, cudaMemcpyHostToDevice, c->stream));
+        c->dev_F_valid = true;
+    }
     if (n_steps > 0) {
         ls_params q = *p;
         q.chained = 0;   // the staging field was just overwritten
@@ -597,30 +604,36 @@ ls_status ls_step_snapshots(ls_ctx* c, void* phi, const void* F, const ls_params
     if ((st = ensure_field(c, &c->snap[1])) != LS_OK) return st;
     ls_params q = *p;
     int k = 0;   // snapshots taken
-    for (int s = 0; s < n_steps; ++s) {
+    cudaError_t ce = cudaSuccess;
+    const char* what = "";
+    auto ck = [&](cudaError_t e, const char* w) { if (ce == cudaSuccess && e != cudaSuccess) { ce = e; what = w; } return e == cudaSuccess; };
+    // On any failure: leave the loop, then ALWAYS drain both streams (copies into the caller's host_out may be in flight)
+    // and report how many snapshots were written before returning the first error.
+    for (int s = 0; s < n_steps && st == LS_OK && ce == cudaSuccess; ++s) {
         st = c->dtype == LS_F32 ? step_impl<float>(c, (float*)phi, (const float*)F, &q, 1)
                                 : step_impl<double>(c, (double*)phi, (const double*)F, &q, 1);
         if (st != LS_OK) break;
         q.chained = 1;   // same buffer, untouched in between
         if ((s + 1) % every == 0) {
             const int slot = k & 1;
-            if (k >= 2) LS_CK(cudaStreamWaitEvent(c->stream, c->snap_free[slot], 0));   // its last D2H has drained
+            if (k >= 2 && !ck(cudaStreamWaitEvent(c->stream, c->snap_free[slot], 0), "cudaStreamWaitEvent")) break;   // its last D2H has drained
             {
                 ProfScope ps(c, LS_K_COPY);
-                LS_CK(cudaMemcpyAsync(c->snap[slot], phi, bytes, cudaMemcpyDeviceToDevice, c->stream));
+                if (!ck(cudaMemcpyAsync(c->snap[slot], phi, bytes, cudaMemcpyDeviceToDevice, c->stream), "snapshot copy")) break;
             }
-            LS_CK(cudaEventRecord(c->snap_ready[slot], c->stream));
-            LS_CK(cudaStreamWaitEvent(c->copy_stream, c->snap_ready[slot], 0));
-            LS_CK(cudaMemcpyAsync((char*)host_out + (size_t)k * bytes, c->snap[slot], bytes, cudaMemcpyDeviceToHost,
-                                  c->copy_stream));
-            LS_CK(cudaEventRecord(c->snap_free[slot], c->copy_stream));
+            if (!ck(cudaEventRecord(c->snap_ready[slot], c->stream), "cudaEventRecord")) break;
+            if (!ck(cudaStreamWaitEvent(c->copy_stream, c->snap_ready[slot], 0), "cudaStreamWaitEvent")) break;
+            if (!ck(cudaMemcpyAsync((char*)host_out + (size_t)k * bytes, c->snap[slot], bytes, cudaMemcpyDeviceToHost,
+                                    c->copy_stream), "snapshot download")) break;
+            if (!ck(cudaEventRecord(c->snap_free[slot], c->copy_stream), "cudaEventRecord")) break;
             ++k;
         }
     }
     cudaError_t e1 = cudaStreamSynchronize(c->stream), e2 = cudaStreamSynchronize(c->copy_stream);
+    if (n_written) *n_written = k;
+    if (ce != cudaSuccess) return cuda_fail(ce, what);
     if (e1 != cudaSuccess) return cuda_fail(e1, "ls_step_snapshots: cudaStreamSynchronize");
     if (e2 != cudaSuccess) return cuda_fail(e2, "ls_step_snapshots: cudaStreamSynchronize(copy)");
-    if (n_written) *n_written = k;
     return st;
 }
 

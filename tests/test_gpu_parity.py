@@ -308,8 +308,14 @@ def test_step_host_matches_device():
     want, _ = orc.step(w.phi, w.F, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, 3)
     host_phi = w.phi.copy()
     with Ctx(w.shape, w.dtype) as ctx:
+        with pytest.raises(ls.LsError):                     # no F on the device yet
+            ls.ls_step_host(ctx, host_phi, None, p, 1)
         ls.ls_step_host(ctx, host_phi, w.F, p, 3)
-    assert np.array_equal(host_phi, want)
+        assert np.array_equal(host_phi, want)
+        # F is static (R17): the following calls reuse the device copy
+        want2, _ = orc.step(want, w.F, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, 2)
+        ls.ls_step_host(ctx, host_phi, None, p, 2)
+        assert np.array_equal(host_phi, want2)
 
 
 def test_dense_cfg2_steps():
