@@ -570,3 +570,93 @@ def test_step_snapshots_match_oracle_trajectory():
             assert ls.ls_step_snapshots(ctx, d_phi, d_F, p1, 2, 5, host) == 0     # fewer steps than `every`
             assert np.array_equal(d_phi.cpu().numpy(), traj[8])
             assert ls.ls_stats(ctx)[1] == 9
+
+
+# ---------------------------------------------------------------------------------------------
+# Late steps at BASELINE.json's full sizes and lengths (windowed parity, SURVEY.md section 8(c) protocol 3-ii): the GPU runs
+# N - 1 steps alone, the crops of phi^{N-1} are downloaded, one more step follows, and the oracle repeats that ONE step
+# from the GPU's own phi^{N-1} crops.  The incremental rebuild's exactness argument (T^{n+1} inside N^n)
+# is the kind of thing that breaks late (fronts merging in cfg 3, the band reaching the domain faces), not at step 3.
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,total", [(4, 200), (3, 100)])
+def test_full_size_late_step_windowed(cfg, total):
+    w = inputs.config(cfg)
+    n, size, margin = w.nx, 112, 8
+    p0 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, ls.LS_REBUILD_INCREMENTAL, 0)
+    p1 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, ls.LS_REBUILD_INCREMENTAL, 1)
+    with Ctx(w.shape, w.dtype) as ctx:
+        d_phi, d_F = to_dev(w.phi), to_dev(w.F)
+        ls.ls_step(ctx, d_phi, d_F, p0, 1)
+        ls.ls_step(ctx, d_phi, d_F, p1, total - 2)           # phi^{N-1}
+        _, _, N_ids, _ = ls.ls_band_export(ctx)              # band of step N-1: where the front is now
+        NB = n // 8
+        picks = [N_ids[int(q * (len(N_ids) - 1))] for q in (0.03, 0.27, 0.5, 0.74, 0.97)]
+        bz, by, bx = np.unravel_index(N_ids, (NB, NB, NB))
+        face = np.flatnonzero((np.minimum.reduce([bz, by, bx]) == 0) | (np.maximum.reduce([bz, by, bx]) == NB - 1))
+        if len(face):                                        # a brick where the band touches a domain face (cfg 3)
+            picks.append(N_ids[face[len(face) // 2]])
+        centres = [[(c * 8 + 4) for c in np.unravel_index(int(b), (NB, NB, NB))] for b in picks]
+        boxes = _crop_boxes(n, centres, size, margin)
+        prev = [d_phi[tuple(slice(o, o + size) for o in org)].contiguous().cpu().numpy() for org, _, _ in boxes]
+        upd0 = ls.ls_stats(ctx)[0]
+        ls.ls_step(ctx, d_phi, d_F, p1, 1)                    # step N
+        nT, nN, bT, bN = ls.ls_band_counts(ctx)
+        assert ls.ls_stats(ctx)[0] - upd0 == nT + w.iters * nN
+        T_ids, T_w, N_ids, N_w = ls.ls_band_export(ctx)
+        got = [d_phi[tuple(slice(o, o + size) for o in org)].contiguous().cpu().numpy() for org, _, _ in boxes]
+        gamma32 = np.float32(w.gamma)
+        assert float(d_phi.abs().max().item()) <= gamma32
+    checked = 0
+    for (org, lo, hi), phi_c, g in zip(boxes, prev, got):
+        sl = tuple(slice(o, o + size) for o in org)
+        inner = tuple(slice(l, h) for l, h in zip(lo, hi))
+        F_c = np.ascontiguousarray(w.F[sl])
+        want, _ = orc.step(phi_c, F_c, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, 1)
+        assert np.array_equal(g[inner], want[inner]), f"crop at {org}: max err {max_err_dx(g[inner], want[inner], w.dx)} dx"
+        Tm, Nm = orc.band_masks(phi_c, w.gamma)
+        assert np.array_equal(_masks_from_export(T_ids, T_w, NB, org, lo, hi), Tm[inner] != 0)
+        assert np.array_equal(_masks_from_export(N_ids, N_w, NB, org, lo, hi), Nm[inner] != 0)
+        checked += int((Nm[inner] != 0).sum())
+    assert checked > 50000
+
+
+def test_cfg2_step_50_full_grid():
+    """cfg 2 at its full size and length: 49 full-domain advances on the GPU alone, then the 50th compared with ONE
+    oracle advance of the GPU's own phi^49, every point of the 256^3 grid, bit for bit."""
+    w = inputs.config(2)
+    with Ctx(w.shape, w.dtype) as ctx:
+        a, d_F = to_dev(w.phi), to_dev(w.F)
+        b = torch.empty_like(a)
+        for _ in range(49):
+            ls.ls_advance(ctx, a, d_F, w.dt, w.dx, INF, INF, b)
+            a, b = b, a
+        prev = a.cpu().numpy()
+        ls.ls_advance(ctx, a, d_F, w.dt, w.dx, INF, INF, b)
+        got = b.cpu().numpy()
+    want = orc.advance(prev, w.F, None, w.dt, w.dx, INF, INF)
+    assert np.array_equal(got, want)
+    assert np.abs(prev - w.phi).max() > 10 * w.dx            # the front really moved (F >= 0.5, 49 x 0.4 dx)
+
+
+@pytest.mark.parametrize("rebuild", [ls.LS_REBUILD_FULL, ls.LS_REBUILD_INCREMENTAL])
+@pytest.mark.parametrize("cfg,n,steps", [(3, 128, 100), (4, 128, 200)])
+def test_free_running_full_length(cfg, n, steps, rebuild):
+    """BASELINE.json's step counts, free running, on grids the oracle can follow: |T| and |N| of every step and the
+    final field must equal the oracle's (a single flipped band bit anywhere would show in the counts)."""
+    w = inputs.config(cfg, n=n)
+    want_counts = []
+    phi = w.phi
+    for _ in range(steps):
+        Tm, Nm = orc.band_masks(phi, w.gamma)
+        want_counts.append((int(Tm.sum()), int(Nm.sum())))
+        phi, _ = orc.step(phi, w.F, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, 1)
+    got_counts = []
+    with Ctx(w.shape, w.dtype) as ctx:
+        d_phi, d_F = to_dev(w.phi), to_dev(w.F)
+        for s in range(steps):
+            ls.ls_step(ctx, d_phi, d_F, ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild, 1 if s else 0), 1)
+            got_counts.append(ls.ls_band_counts(ctx)[:2])
+        got = d_phi.cpu().numpy()
+    assert got_counts == want_counts
+    assert np.array_equal(got, phi)
+    assert want_counts[-1] != want_counts[0]
