@@ -161,23 +161,27 @@ __global__ void __launch_bounds__(kDilateWarps * 32) k_dilate_items(Geom g, Dila
     const int nprev = INCREMENTAL ? *a.prevCount : 0, nstale = INCREMENTAL ? *a.staleCount : 0;
     const int64_t ncand = INCREMENTAL ? (int64_t)nprev * 7 + nstale : (int64_t)g.nquads;
     const int64_t nwarps = (int64_t)gridDim.x * kDilateWarps;
-    auto tvalid = [&](int q) -> bool { return a.qflagT[q] != 0 && (a.tgate == nullptr || a.tgate[q] != 0); };
+    // T masks are valid for quad q if its flag is set and (incremental builds) it lay in the previous band.  Both
+    // bytes are loaded unconditionally (no dependent branch between them): what this kernel waits for is the flags.
+    const uint8_t* gate = a.tgate != nullptr ? a.tgate : a.qflagT;
+    auto tvalid = [&](bool inside, int q) -> unsigned { return inside ? ((a.qflagT[q] != 0) & (gate[q] != 0) ? 1u : 0u) : 0u; };
     // A warp turn takes 32 consecutive candidates: each lane resolves one (which quad, does another candidate own
-    // it, can it hold an N point at all) with its flag loads in flight together; the quads that need work are
-    // then processed one after the other by the whole warp.
+    // it, which of the quad and its six face neighbours hold valid T masks) with its flag loads in flight together;
+    // the quads that can hold an N point are then processed one after the other by the whole warp.
     for (int64_t w0 = ((int64_t)blockIdx.x * kDilateWarps + wib) * 32; w0 < ncand; w0 += nwarps * 32) {
-    int mine = -1;
+    int mine = -1, my_x = 0, my_y = 0, my_z = 0;
+    unsigned my_valid = 0;   // bit 0: the quad itself, bits 1..6: its -x, +x, -y, +y, -z, +z neighbour
     {
         const int64_t wid = w0 + lane;
         int c = -1;
         if (wid < ncand) c = INCREMENTAL ? candidate_quad(g, a, wid, nprev, nstale) : (int)wid;
         if (c >= 0) {
             const int cx = c % g.NQx, cy = (c / g.NQx) % g.NBy, cz = c / szq;
-            bool any = tvalid(c);
-            any = any || (cx > 0 && tvalid(c - sxq)) || (cx < g.NQx - 1 && tvalid(c + sxq));
-            any = any || (cy > 0 && tvalid(c - syq)) || (cy < g.NBy - 1 && tvalid(c + syq));
-            any = any || (cz > 0 && tvalid(c - szq)) || (cz < g.NBz - 1 && tvalid(c + szq));
-            if (any) {
+            my_x = cx; my_y = cy; my_z = cz;
+            my_valid = tvalid(true, c) | (tvalid(cx > 0, c - sxq) << 1) | (tvalid(cx < g.NQx - 1, c + sxq) << 2) |
+                       (tvalid(cy > 0, c - syq) << 3) | (tvalid(cy < g.NBy - 1, c + syq) << 4) |
+                       (tvalid(cz > 0, c - szq) << 5) | (tvalid(cz < g.NBz - 1, c + szq) << 6);
+            if (my_valid) {
                 mine = c;
             } else {
                 // no T point in reach: the quad is outside N.  Its masks are already zero unless it was in the
@@ -197,12 +201,11 @@ __global__ void __launch_bounds__(kDilateWarps * 32) k_dilate_items(Geom g, Dila
     const int src_lane = __ffs(todo) - 1;
     todo &= todo - 1;
     const int c = __shfl_sync(0xffffffffu, mine, src_lane);
+    const int qx = __shfl_sync(0xffffffffu, my_x, src_lane), by = __shfl_sync(0xffffffffu, my_y, src_lane);
+    const int bz = __shfl_sync(0xffffffffu, my_z, src_lane);
+    const unsigned vm = __shfl_sync(0xffffffffu, my_valid, src_lane);
     __syncwarp();   // the staging of the previous quad has been copied out
-    const int qx = c % g.NQx, by = (c / g.NQx) % g.NBy, bz = c / szq;
-    const bool vs = tvalid(c);
-    const bool vxm = qx > 0 && tvalid(c - sxq), vxp = qx < g.NQx - 1 && tvalid(c + sxq);
-    const bool vym = by > 0 && tvalid(c - syq), vyp = by < g.NBy - 1 && tvalid(c + syq);
-    const bool vzm = bz > 0 && tvalid(c - szq), vzp = bz < g.NBz - 1 && tvalid(c + szq);
+    const bool vs = vm & 1u, vxm = vm & 2u, vxp = vm & 4u, vym = vm & 8u, vyp = vm & 16u, vzm = vm & 32u, vzp = vm & 64u;
     const int j = lane >> 3, lz = lane & 7;   // brick of the quad, word of the brick
     const uint64_t w = vs ? a.tmask[(int64_t)c * 32 + lane] : 0ull;
     uint64_t n = w | ((w << 1) & ~COL0) | ((w >> 1) & ~COL7) | (w << 8) | (w >> 8);
@@ -303,37 +306,43 @@ __global__ void __launch_bounds__(kDilateWarps * 32) k_dilate_items(Geom g, Dila
         if (j == 0) tb[64 + lz] = (unsigned char)E0;
         if (j == 3) tb[72 + lz] = (unsigned char)E7;
         __syncwarp();
+        // Per tile row (y, z): which sectors are needed.  Lanes 0..31 take the 64 quad rows two at a time (z = lane / 4,
+        // y = 2 (lane % 4) + {0, 1}); then one halo row each: y = -1, y = 8 (read by the quad row next to them), z = -1,
+        // z = 8 (corner rows are never read).  Pieces outside the domain are never needed (edge replicate patches them).
         uint8_t* need_out = a.qneed + (int64_t)c * kNeedBytes;
-        for (int r = lane; r < 100; r += 32) {
-            const int y = r % 10 - 1, z = r / 10 - 1;
-            const bool yin = y >= 0 && y < 8, zin = z >= 0 && z < 8;
-            unsigned need = 0;
-            if (yin && zin) {
+        unsigned xclip = 0x3fu;   // sectors of a row that lie inside the domain in x
+        if (qx == 0) xclip &= ~1u;
 #pragma unroll
-                for (int jj = 0; jj < 4; ++jj) need |= (((unsigned)tb[jj * 8 + z] >> y) & 1u) << (1 + jj);
-                need |= ((unsigned)tb[64 + z] >> y) & 1u;
-                need |= (((unsigned)tb[72 + z] >> y) & 1u) << 5;
-            } else if (zin) {   // a halo row in y: read by the quad row next to it
+        for (int ch = 0; ch < 5; ++ch)
+            if (qx * 32 + ch * 8 >= g.nx) xclip &= ~(2u << ch);
+        {
+            const int z = lane >> 2, y0 = (lane & 3) * 2;
+            const unsigned d0 = tb[z], d1 = tb[8 + z], d2 = tb[16 + z], d3 = tb[24 + z], e0 = tb[64 + z], e7 = tb[72 + z];
+            const unsigned r0 = tb[32 + z], r1 = tb[40 + z], r2 = tb[48 + z], r3 = tb[56 + z];
+            const bool zin = bz * 8 + z < g.nz;
 #pragma unroll
-                for (int jj = 0; jj < 4; ++jj) need |= (((unsigned)tb[32 + jj * 8 + z] >> (y < 0 ? 0 : 7)) & 1u) << (1 + jj);
-            } else if (yin) {   // a halo row in z (corner rows are never read)
-#pragma unroll
-                for (int jj = 0; jj < 4; ++jj) need |= (((unsigned)tb[32 + jj * 8 + (z < 0 ? 0 : 7)] >> y) & 1u) << (1 + jj);
+            for (int k = 0; k < 2; ++k) {
+                const int y = y0 + k;
+                unsigned need = ((e0 >> y) & 1u) | (((d0 >> y) & 1u) << 1) | (((d1 >> y) & 1u) << 2) | (((d2 >> y) & 1u) << 3) |
+                                (((d3 >> y) & 1u) << 4) | (((e7 >> y) & 1u) << 5);
+                if (!zin || by * 8 + y >= g.ny) need = 0;
+                need_out[(z + 1) * 10 + (y + 1)] = (uint8_t)(need & xclip);
+                const unsigned own = ((r0 >> y) & 1u) | (((r1 >> y) & 1u) << 1) | (((r2 >> y) & 1u) << 2) | (((r3 >> y) & 1u) << 3);
+                need_out[112 + z * 8 + y] = (uint8_t)own;
             }
+        }
+        {
+            const int kind = lane >> 3, i = lane & 7;   // 0: y = -1, 1: y = 8 (i = z);  2: z = -1, 3: z = 8 (i = y)
+            const int zr = kind < 2 ? i : (kind == 2 ? 0 : 7);              // the layer whose rows read this halo row
+            const int sh = kind < 2 ? (kind == 0 ? 0 : 7) : i;              // the row of that layer which does
+            unsigned need = 0;
+#pragma unroll
+            for (int jj = 0; jj < 4; ++jj) need |= (((unsigned)tb[32 + jj * 8 + zr] >> sh) & 1u) << (1 + jj);
+            const int y = kind < 2 ? (kind == 0 ? -1 : 8) : i, z = kind < 2 ? i : (kind == 2 ? -1 : 8);
             const int gy = by * 8 + y, gz = bz * 8 + z;
             if (gy < 0 || gy >= g.ny || gz < 0 || gz >= g.nz) need = 0;
-            if (qx == 0) need &= ~1u;
-#pragma unroll
-            for (int ch = 0; ch < 5; ++ch)
-                if (qx * 32 + ch * 8 >= g.nx) need &= ~(2u << ch);
-            need_out[r] = (uint8_t)need;
-        }
-        for (int r = lane; r < 64; r += 32) {
-            const int y = r & 7, z = r >> 3;
-            unsigned own = 0;
-#pragma unroll
-            for (int jj = 0; jj < 4; ++jj) own |= (((unsigned)tb[32 + jj * 8 + z] >> y) & 1u) << jj;
-            need_out[112 + r] = (uint8_t)own;
+            need_out[(z + 1) * 10 + (y + 1)] = (uint8_t)(need & xclip);
+            if (lane < 4) need_out[(lane >> 1) * 90 + (lane & 1) * 9] = 0;   // the four corner rows
         }
     }
     // does an N point sit on the quad's low-x / high-x face?  (the band kernels load that x halo only then)

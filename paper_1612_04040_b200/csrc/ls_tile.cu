@@ -82,17 +82,22 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// (with a suspend-time hint the hardware parks the waiting warp; a bare try_wait loop returns at once and spins, and the
+// spinning takes issue slots from the warps of the other CTAs on the SM: 22 M of 73 M warp instructions of a sweep, measured)
+#ifndef LS_WAIT_HINT_NS
+#define LS_WAIT_HINT_NS 20000u
+#endif
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
         "LS_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
         "@p bra LS_DONE;\n"
         "bra LS_WAIT;\n"
         "LS_DONE:\n"
         "}\n" ::"r"(bar),
-        "r"(parity)
+        "r"(parity), "r"(LS_WAIT_HINT_NS)
         : "memory");
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
@@ -238,7 +243,7 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_M, const __grid_constant__ CU
             const __grid_constant__ CUtensorMap tm_F, T* __restrict__ dst, Geom g, StencilParams<T> pa,
             StencilParams<T> pr, TileArgs a) {
     static_assert(K == 1 || (K == 2 && !ADV && NCW == 8 && NPW == 1), "K = 2: two reinit sweeps, 256 consumers");
-    static_assert(K != 1 || NPW == STAGES, "K = 1: one producer warp per stage");
+    static_assert(K != 1 || NPW == STAGES || NPW == 1, "K = 1: one producer warp per stage, or one for all stages");
     using S = Stage<T, K, ADV>;
     using TL = Tile<T, K>;
     constexpr int NC = NCW * 32, XW = S::XW;
@@ -247,8 +252,9 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_M, const __grid_constant__ CU
     const uint32_t smem_base = smem_u32(smem);
     // after the stages: T staging of EMIT_T (2 x 512 B: one byte per item position), then the mbarriers
     // (full[STAGES], empty[STAGES])
+    constexpr int TS_BYTES = EMIT_T ? 1024 : 0;
     unsigned char* tstage = smem + STAGES * S::BYTES;
-    const uint32_t bar_full = smem_base + STAGES * S::BYTES + 1024, bar_empty = bar_full + 8 * STAGES;
+    const uint32_t bar_full = smem_base + STAGES * S::BYTES + TS_BYTES, bar_empty = bar_full + 8 * STAGES;
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < STAGES; ++s) { mbar_init(bar_full + 8 * s, K == 1 ? 33 : 1); mbar_init(bar_empty + 8 * s, NCW); }
@@ -315,11 +321,14 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_M, const __grid_constant__ CU
         // the consumers work through the other stages.  Tiles cost between 1 and 512 items, so any tile reserved
         // early is load imbalance at the end of the launch: with tickets drawn in chunks and one chunk ahead, two
         // thirds of the list were handed out in the first microsecond and the slowest CTA ran 1.4x the mean.
-        const int slot = warp - NCW;
-        const uint32_t st = smem_base + slot * S::BYTES, bar = bar_full + 8 * slot;
-        Hdr* const h = reinterpret_cast<Hdr*>(smem + slot * S::BYTES + S::OFF_HDR);
+        // NPW == STAGES: warp p owns stage p.  NPW == 1: one warp fills the stages in turn (smaller CTAs, more of them
+        // per SM: what hides the consumers' latencies is the number of consumer warps on the SM).
         int issued = 0;
         for (;;) {
+            const int slot = NPW == 1 ? issued % STAGES : warp - NCW;
+            const int fill = NPW == 1 ? issued / STAGES : issued;          // fills of this stage so far
+            const uint32_t st = smem_base + slot * S::BYTES, bar = bar_full + 8 * slot;
+            Hdr* const h = reinterpret_cast<Hdr*>(smem + slot * S::BYTES + S::OFF_HDR);
             int idx = 0;
             if (lane == 0) idx = (int)atomicAdd(a.ticket, 1u);
             idx = __shfl_sync(0xffffffffu, idx, 0);
@@ -340,7 +349,7 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_M, const __grid_constant__ CU
             const T* qsrc = src + org;
             const uint16_t* item_src = a.items + (int64_t)quad * kItemsPerQuad;
             // ---- the stage's previous tenant has been consumed ----
-            if (issued >= 1) mbar_wait(bar_empty + 8 * slot, (uint32_t)((issued - 1) & 1));
+            if (fill >= 1) mbar_wait(bar_empty + 8 * slot, (uint32_t)((fill - 1) & 1));
             // ---- fire ----
             if (lane == 0) {
                 h->quad = quad;
@@ -393,13 +402,17 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_M, const __grid_constant__ CU
             cp_async_arrive(bar);
             ++issued;
         }
-        // sentinel: this stage gets no more work
-        if (issued >= 1) mbar_wait(bar_empty + 8 * slot, (uint32_t)((issued - 1) & 1));
-        if (lane == 0) {
-            reinterpret_cast<Hdr*>(smem + slot * S::BYTES + S::OFF_HDR)->quad = -1;
-            mbar_expect_tx(bar_full + 8 * slot, 0);
+        // sentinel: this stage gets no more work (NPW == 1: nor do the others, the consumers stop at the first one)
+        {
+            const int slot = NPW == 1 ? issued % STAGES : warp - NCW;
+            const int fill = NPW == 1 ? issued / STAGES : issued;
+            if (fill >= 1) mbar_wait(bar_empty + 8 * slot, (uint32_t)((fill - 1) & 1));
+            if (lane == 0) {
+                reinterpret_cast<Hdr*>(smem + slot * S::BYTES + S::OFF_HDR)->quad = -1;
+                mbar_expect_tx(bar_full + 8 * slot, 0);
+            }
+            cp_async_arrive(bar_full + 8 * slot);
         }
-        cp_async_arrive(bar_full + 8 * slot);
         // self-resetting scheduler: the last producer warp to finish fetching zeroes the counters for the next launch
         if (lane == 0) {
             __threadfence();
@@ -503,9 +516,9 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_M, const __grid_constant__ CU
         phases ^= 1u << slot;
         Hdr* hp = reinterpret_cast<Hdr*>(st + S::OFF_HDR);
         const int quad = hp->quad;
-        if (quad < 0) {   // K = 1: this stage's producer is done; K = 2: the only producer is
+        if (quad < 0) {   // one producer per stage: this stage's producer is done; a single producer: all work is done
             alive &= ~(1u << slot);
-            if (K > 1 || alive == 0) break;
+            if (NPW == 1 || alive == 0) break;
             next_slot();
             continue;
         }
@@ -839,11 +852,18 @@ struct Maps { CUtensorMap M, H, F; };
 template <typename T, bool ADV, int K, bool CLAMP, bool RESIDUAL, bool EMIT_T>
 void launch_variant(const Maps& m, T* dst, const Geom& g, const StencilParams<T>& pa, const StencilParams<T>& pr,
                     const TileArgs& a, cudaStream_t s) {
+#ifndef LS_K1_STAGES
+#define LS_K1_STAGES 2
+#endif
+#ifndef LS_K1_NPW
+#define LS_K1_NPW 0   // 0: one producer warp per stage
+#endif
     constexpr int NCW = K > 1 ? 8 : 4;
-    constexpr int STAGES = (K > 1 || ADV || sizeof(T) == 8) ? 2 : 3;
-    constexpr int NPW = K > 1 ? 1 : STAGES;   // K = 1: one gather warp per stage; K = 2: one lane issuing TMA boxes
+    constexpr int STAGES = (K > 1 || ADV || sizeof(T) == 8) ? 2 : LS_K1_STAGES;
+    // K = 1: gather warps (one per stage, or one for all stages); K = 2: one lane issuing TMA boxes
+    constexpr int NPW = K > 1 ? 1 : (LS_K1_NPW ? LS_K1_NPW : STAGES);
     using S = Stage<T, K, ADV>;
-    const size_t shm = (size_t)STAGES * S::BYTES + 1024 + 16 * STAGES;
+    const size_t shm = (size_t)STAGES * S::BYTES + (EMIT_T ? 1024 : 0) + 16 * STAGES;
     auto kern = k_band_tile<T, ADV, K, CLAMP, RESIDUAL, EMIT_T, STAGES, NCW, NPW>;
     // (the grid is sized once per process for the device current at the first launch: every B200 is alike)
     static const int grid = persistent_grid(kern, (NCW + NPW) * 32, shm);

@@ -660,3 +660,49 @@ def test_free_running_full_length(cfg, n, steps, rebuild):
     assert got_counts == want_counts
     assert np.array_equal(got, phi)
     assert want_counts[-1] != want_counts[0]
+
+
+def test_cfg5_runs_to_its_stopping_rule():
+    """cfg 5 as BASELINE.json states it: 512^3 fp64, reinit 'solved to steady state' (R13: max_N |d^k - d^{k-1}|
+    < 1e-10).  The GPU iterates alone to the stopping rule; the oracle certifies the fixed point: ONE oracle iteration from
+    crops of the converged state moves no well-inside band point by 1e-10 or more, and repeats the GPU's own next sweep bit
+    for bit.  (About 2.5e5 sweeps, 20 s of GPU time.)  Writes iterations / residual / seconds to
+    gpurun_out/cfg5_converged.json."""
+    import json
+    import os
+    import time
+    w = inputs.config(5)
+    n, size = w.nx, 128
+    with Ctx(w.shape, w.dtype) as ctx:
+        d_phi = to_dev(w.phi)
+        d = torch.empty_like(d_phi)
+        ls.ls_build_band(ctx, d_phi, w.dx, w.gamma)
+        nT, nN, _, _ = ls.ls_band_counts(ctx)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        k, r, conv = ls.ls_reinit_tol(ctx, d, d_phi, w.dtau, w.dx, w.gamma, w.tol, 6_000_000, 2000)
+        torch.cuda.synchronize()
+        secs = time.perf_counter() - t0
+        os.makedirs("gpurun_out", exist_ok=True)
+        with open("gpurun_out/cfg5_converged.json", "w") as f:
+            json.dump({"workload": "cfg5 512^3 fp64", "tol": w.tol, "check_every": 2000, "iterations": k, "residual": r,
+                       "converged": conv, "seconds": secs, "N_points": nN, "us_per_sweep": secs / max(k, 1) * 1e6}, f)
+        assert conv and r < w.tol and k % 2000 == 0
+        got = d.cpu().numpy()
+        d2 = torch.empty_like(d)
+        ls.ls_reinit(ctx, d2, d, w.dtau, w.dx, w.gamma, 1)      # the GPU's own next sweep from the converged state
+        nxt = d2.cpu().numpy()
+    boxes = _crop_boxes(n, [[0.5 * n, 0.25 * n, n / 3], [0.5 * n, 0.75 * n, 2 * n / 3], [0.5 * n, 0.0, 0.0]], size, 2)
+    checked = 0
+    for org, lo, hi in boxes:
+        sl = tuple(slice(o, o + size) for o in org)
+        inner = tuple(slice(l, h) for l, h in zip(lo, hi))
+        _, Nm = orc.band_masks(np.ascontiguousarray(w.phi[sl]), w.gamma)       # the tube N of phi^0 (R25)
+        c = np.ascontiguousarray(got[sl])
+        one, _ = orc.reinit_iter(c, Nm, w.dtau, w.dx)
+        # clamped rim values (eq. 10 ran at the end) feed their neighbours: certify two cells inside the clamp
+        well = (Nm[inner] != 0) & (np.abs(c[inner]) < w.gamma - 2 * w.dx)
+        assert np.abs(one[inner] - c[inner])[well].max() < w.tol
+        assert np.array_equal(np.clip(one, -w.gamma, w.gamma)[inner][well], nxt[sl][inner][well])
+        checked += int(well.sum())
+    assert checked > 100000
