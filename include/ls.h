@@ -53,7 +53,9 @@ typedef enum {
     LS_REBUILD_FULL = 0,        /* scan every grid point each step, as the paper does */
     LS_REBUILD_INCREMENTAL = 1  /* exact: after the first step phi is clamped (eq. 10), so
                                    T^{n+1} is a subset of N^n and only the bricks of N^n
-                                   are re-classified — fused into the last reinit sweep */
+                                   are re-classified — fused into the launch that writes phi^{n+1}: the
+                                   last reinit sweep, or (iters even or 0) the band copy that moves the
+                                   result; either way no whole-grid pass after the first step */
 } ls_rebuild;
 
 /* Parameters of one narrow-band step (Steps 1-3). */
@@ -190,7 +192,7 @@ ls_status ls_profile_enable(ls_ctx* ctx, int32_t on);
 ls_status ls_profile_read(ls_ctx* ctx, int32_t kind, double* ms_total, int64_t* launches);
 ls_status ls_profile_reset(ls_ctx* ctx);
 
-/* Device self-check of the fp32 arithmetic: the band kernels evaluate two points per lane with packed
+/* DIAGNOSTIC, not part of the path: device self-check of the fp32 arithmetic: the band kernels evaluate two points per lane with packed
  * FADD2 / FMUL2 / FFMA2 instructions and hand-sequenced correctly rounded sqrt / divide; this runs both
  * that path and the plain scalar IEEE path (eq. 3-8 and eq. 12-13) on `n` pairs of seeded random 7-point
  * stencils (band-like values, arbitrary bit patterns, zeros, flat patches) on the current device and

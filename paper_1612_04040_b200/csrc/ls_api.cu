@@ -688,7 +688,8 @@ ls_status ls_selftest_math(void* cuda_stream, uint64_t seed, int64_t n, double d
     cudaFree(d);
     if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(e, "ls_selftest_math"); }
     const unsigned long long h = out.n[0];
-    if (h && getenv("LS_SELFTEST_VERBOSE")) {   // first differing sample: stencils (zm ym xm c xp yp zp) x2, F, scalar / packed results
+#ifdef LS_DEBUG
+    if (h) {   // first differing sample: stencils (zm ym xm c xp yp zp) x2, F, scalar / packed results
         std::fprintf(stderr, "ls_selftest_math: %llu results differ; first sample:\n", h);
         for (int k = 0; k < 32; ++k) {
             unsigned bits;
@@ -696,6 +697,7 @@ ls_status ls_selftest_math(void* cuda_stream, uint64_t seed, int64_t n, double d
             std::fprintf(stderr, "  [%2d] %.9g (0x%08x)\n", k, out.v[k], bits);
         }
     }
+#endif
     *mismatches = (int64_t)h;
     return LS_OK;
 }

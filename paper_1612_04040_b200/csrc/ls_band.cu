@@ -1,8 +1,8 @@
 // ls_band.cu — Step 1: tubes T (eq. 6) and N (eq. 11).
 //
 // Kernels
-//   k_classify        whole-grid sweep, one CTA per quad (32x8x8 points), 128-bit coalesced
-//                     loads; T bits are assembled into brick mask words with warp REDUX (no atomics).
+//   k_classify        whole-grid sweep, one CTA per x-row of quads (32x8x8 points each), 128-bit
+//                     coalesced loads; T bits are assembled into brick mask words with warp REDUX (no atomics).
 //   k_dilate_items    one WARP per candidate quad: lane (j, lz) builds N word lz of brick j from its own T
 //                     word, its neighbours' words by shuffle, and the facing bit planes of the six
 //                     neighbour quads (eq. 11, R6); then the quad's item list (ls_internal.h) by a warp
@@ -27,60 +27,74 @@ template <typename T> __device__ __forceinline__ T absval(T v);
 template <> __device__ __forceinline__ float absval<float>(float v) { return fabsf(v); }
 template <> __device__ __forceinline__ double absval<double>(double v) { return fabs(v); }
 
-// One CTA = one quad = 32(x) x 8(y) x 8(z) points.  Warp w owns z-layer w; lane l owns the 4 consecutive
-// x cells x4 = l&7 of row y = (l>>3) + 4h, h = 0,1.  With VEC the 4 cells are one 128-bit load and a warp
-// load covers 4 full 128-byte lines.  Writes all 32 mask words of the quad (zeros included) and its flag.
+// One CTA = one x-row of quads (by, bz), a segment of `qper` of them; one quad = 32(x) x 8(y) x 8(z) points.  Warp w owns
+// z-layer w; lane l owns the 4 consecutive x cells x4 = l&7 of row y = (l>>3) + 4h, h = 0,1.  With VEC the 4 cells are one
+// 128-bit load and a warp load covers 4 full 128-byte lines.  The CTA walks its quads along x, so the coordinates and row
+// pointers are set up once and a quad costs two loads, eight compares and two REDUX per lane (round 1 launched one CTA per
+// quad: the set-up made it issue bound at 55 % of the copy bandwidth).  Writes all 32 mask words of every quad (zeros
+// included) and its flag.
 template <typename T, bool VEC>
-__global__ void __launch_bounds__(256) k_classify(const T* __restrict__ phi, Geom g, T gamma,
+__global__ void __launch_bounds__(256) k_classify(const T* __restrict__ phi, Geom g, T gamma, int qper,
                                                   uint64_t* __restrict__ tmask, uint8_t* __restrict__ qflagT) {
-    __shared__ uint32_t half_words[8][4][2];  // [lz][brick in quad][low/high 32 bits]
-    const int quad = blockIdx.x;
-    const int qx = quad % g.NQx;
-    const int by = (quad / g.NQx) % g.NBy;
-    const int bz = quad / (g.NQx * g.NBy);
+    __shared__ uint32_t half_words[2][8][4][2];  // [parity of the quad][lz][brick in quad][low/high 32 bits]
+    const int nseg = (g.NQx + qper - 1) / qper;
+    const int seg = blockIdx.x % nseg, rowid = blockIdx.x / nseg;   // rowid = bz * NBy + by
+    const int by = rowid % g.NBy, bz = rowid / g.NBy;
     const int lane = threadIdx.x & 31, lz = threadIdx.x >> 5;
     const int k = bz * 8 + lz;
     const int x4 = lane & 7;
-    const int i0 = qx * 32 + x4 * 4;
     const int q = x4 >> 1;                                  // brick of the quad this lane feeds
     const unsigned group = 0x03030303u << (2 * q);          // the 8 lanes feeding the same 32-bit half
-
+    const T* row[2];
+    bool row_ok[2];
+    unsigned shift[2];
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
         const int ly = (lane >> 3) + 4 * h;
         const int j = by * 8 + ly;
-        unsigned bits = 0;
-        if (k < g.nz && j < g.ny && i0 < g.nx) {
-            const T* row = phi + g.idx(0, j, k);
-            if (VEC) {  // nx % 4 == 0 here, so i0 + 3 < nx
-                if (sizeof(T) == 4) {
-                    const float4 v = __ldg(reinterpret_cast<const float4*>(row + i0));
-                    bits = (absval<T>((T)v.x) < gamma ? 1u : 0u) | (absval<T>((T)v.y) < gamma ? 2u : 0u) |
-                           (absval<T>((T)v.z) < gamma ? 4u : 0u) | (absval<T>((T)v.w) < gamma ? 8u : 0u);
-                } else {
-                    const double2 a = __ldg(reinterpret_cast<const double2*>(row + i0));
-                    const double2 b = __ldg(reinterpret_cast<const double2*>(row + i0 + 2));
-                    bits = (absval<T>((T)a.x) < gamma ? 1u : 0u) | (absval<T>((T)a.y) < gamma ? 2u : 0u) |
-                           (absval<T>((T)b.x) < gamma ? 4u : 0u) | (absval<T>((T)b.y) < gamma ? 8u : 0u);
-                }
-            } else {
-#pragma unroll
-                for (int e = 0; e < 4; ++e)
-                    if (i0 + e < g.nx && absval<T>(__ldg(row + i0 + e)) < gamma) bits |= 1u << e;
-            }
-        }
-        // bit position inside the 32-bit half: row (ly & 3), columns (x4 & 1)*4 ..
-        const unsigned v = bits << ((ly & 3) * 8 + (x4 & 1) * 4);
-        const unsigned r = __reduce_or_sync(group, v);
-        if ((lane & 0x19) == 0) half_words[lz][q][h] = r;   // lanes 0,2,4,6: first lane of each group
+        row_ok[h] = k < g.nz && j < g.ny;
+        row[h] = phi + g.idx(0, row_ok[h] ? j : 0, row_ok[h] ? k : 0);
+        shift[h] = (ly & 3) * 8 + (x4 & 1) * 4;             // bit position inside the 32-bit half: row (ly & 3), columns (x4 & 1)*4 ..
     }
-    __syncthreads();
-    if (threadIdx.x < 32) {
-        const int qq = threadIdx.x >> 3, z = threadIdx.x & 7;
-        const uint64_t word = (uint64_t)half_words[z][qq][0] | ((uint64_t)half_words[z][qq][1] << 32);
-        const unsigned nz_lanes = __ballot_sync(0xffffffffu, word != 0);
-        tmask[(int64_t)quad * 32 + threadIdx.x] = word;
-        if (threadIdx.x == 0) qflagT[quad] = nz_lanes ? 1 : 0;
+    const int q0 = seg * qper, q1 = min(g.NQx, q0 + qper);
+    for (int qx = q0; qx < q1; ++qx) {
+        const int i0 = qx * 32 + x4 * 4;
+        const int par = (qx - q0) & 1;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            unsigned bits = 0;
+            if (row_ok[h] && i0 < g.nx) {
+                if (VEC) {  // nx % 4 == 0 here, so i0 + 3 < nx
+                    if (sizeof(T) == 4) {
+                        const float4 v = __ldg(reinterpret_cast<const float4*>(row[h] + i0));
+                        bits = (absval<T>((T)v.x) < gamma ? 1u : 0u) | (absval<T>((T)v.y) < gamma ? 2u : 0u) |
+                               (absval<T>((T)v.z) < gamma ? 4u : 0u) | (absval<T>((T)v.w) < gamma ? 8u : 0u);
+                    } else {
+                        const double2 a = __ldg(reinterpret_cast<const double2*>(row[h] + i0));
+                        const double2 b = __ldg(reinterpret_cast<const double2*>(row[h] + i0 + 2));
+                        bits = (absval<T>((T)a.x) < gamma ? 1u : 0u) | (absval<T>((T)a.y) < gamma ? 2u : 0u) |
+                               (absval<T>((T)b.x) < gamma ? 4u : 0u) | (absval<T>((T)b.y) < gamma ? 8u : 0u);
+                    }
+                } else {
+#pragma unroll
+                    for (int e = 0; e < 4; ++e)
+                        if (i0 + e < g.nx && absval<T>(__ldg(row[h] + i0 + e)) < gamma) bits |= 1u << e;
+                }
+            }
+            const unsigned r = __reduce_or_sync(group, bits << shift[h]);
+            if ((lane & 0x19) == 0) half_words[par][lz][q][h] = r;   // lanes 0,2,4,6: first lane of each group
+        }
+        __syncthreads();   // (the other parity's words were read before the previous barrier's successor: see below)
+        if (threadIdx.x < 32) {
+            // warp 0 assembles the quad's 32 words; it reaches the next barrier only after these reads, and the words of
+            // this parity are next written two quads later, after that barrier
+            const int qq = threadIdx.x >> 3, z = threadIdx.x & 7;
+            const uint64_t word = (uint64_t)half_words[par][z][qq][0] | ((uint64_t)half_words[par][z][qq][1] << 32);
+            const unsigned nz_lanes = __ballot_sync(0xffffffffu, word != 0);
+            const int64_t quad = (int64_t)rowid * g.NQx + qx;
+            tmask[quad * 32 + threadIdx.x] = word;
+            if (threadIdx.x == 0) qflagT[quad] = nz_lanes ? 1 : 0;
+        }
     }
 }
 
@@ -561,10 +575,15 @@ __global__ void __launch_bounds__(256) k_export_scatter(ExportArgs a, Geom g, in
 template <typename T>
 void launch_classify(const T* phi, const Geom& g, T gamma, BandBuffers& bb, cudaStream_t s, int64_t* launches) {
     const bool vec = (g.nx % 4 == 0) && ((reinterpret_cast<uintptr_t>(phi) & 15) == 0);
+    // one CTA per x-row of quads, split into segments while that leaves fewer CTAs than a few waves of the GPU
+    const int rows = g.NBy * g.NBz;
+    int qper = g.NQx;
+    while (qper > 4 && (int64_t)rows * ((g.NQx + qper - 1) / qper) < (int64_t)sm_count() * 16) qper = (qper + 1) / 2;
+    const unsigned grid = (unsigned)(rows * ((g.NQx + qper - 1) / qper));
     if (vec)
-        k_classify<T, true><<<(unsigned)g.nquads, 256, 0, s>>>(phi, g, gamma, bb.tmask[bb.tb], bb.qflagT[bb.tb]);
+        k_classify<T, true><<<grid, 256, 0, s>>>(phi, g, gamma, qper, bb.tmask[bb.tb], bb.qflagT[bb.tb]);
     else
-        k_classify<T, false><<<(unsigned)g.nquads, 256, 0, s>>>(phi, g, gamma, bb.tmask[bb.tb], bb.qflagT[bb.tb]);
+        k_classify<T, false><<<grid, 256, 0, s>>>(phi, g, gamma, qper, bb.tmask[bb.tb], bb.qflagT[bb.tb]);
     bb.tvalid_all = true;
     if (launches) *launches += 1;
 }

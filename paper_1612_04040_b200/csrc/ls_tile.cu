@@ -24,6 +24,8 @@
 // tile path cannot address (nx not a multiple of 4, unaligned fields).
 #include <cuda.h>
 
+#include <cstring>
+
 #include "ls_internal.h"
 #include "ls_math.cuh"
 
@@ -255,6 +257,16 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_M, const __grid_constant__ CU
     constexpr int TS_BYTES = EMIT_T ? 1024 : 0;
     unsigned char* tstage = smem + STAGES * S::BYTES;
     const uint32_t bar_full = smem_base + STAGES * S::BYTES + TS_BYTES, bar_empty = bar_full + 8 * STAGES;
+    // Small bands (cfg 1, the paper's 101^3): most CTAs of the persistent grid have nothing to do.  They leave before
+    // touching shared memory — only the scheduler's "producer warps done" count must still see them.
+    const int count = *a.count;
+    if ((int)blockIdx.x >= count) {
+        if (tid == 0) {
+            __threadfence();
+            if (atomicAdd(a.ticket + 1, (unsigned)NPW) + NPW == gridDim.x * NPW) { a.ticket[0] = 0u; a.ticket[1] = 0u; }
+        }
+        return;
+    }
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < STAGES; ++s) { mbar_init(bar_full + 8 * s, K == 1 ? 33 : 1); mbar_init(bar_empty + 8 * s, NCW); }
@@ -266,7 +278,6 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_M, const __grid_constant__ CU
     // bit patterns the last kernel left in shared memory (a NaN would send a lane down the scalar slow path).
     for (int i = tid; i < STAGES * S::BYTES / 16; i += (NCW + NPW) * 32) reinterpret_cast<uint4*>(smem)[i] = make_uint4(0u, 0u, 0u, 0u);
     __syncthreads();
-    const int count = *a.count;
 
     if (warp >= NCW && K == 1) {
         // ------------------------------ producer, K = 1: sparse gather ------------------------------
@@ -697,108 +708,6 @@ k_band_tile(const __grid_constant__ CUtensorMap tm_M, const __grid_constant__ CU
     }
 }
 
-// ---------------------------------------------------------------------------------------------
-// Direct variant of a K = 1 reinit sweep: no shared-memory tile.  One WARP per quad and turn; lane l evaluates
-// items l, l+32, ... of the quad's list, reading its stencil straight from the field through L1 (the rows a
-// quad touches stay resident while the warp walks the list) and writing its 16 bytes.  Latency is hidden by
-// occupancy alone.  Same arithmetic, same writes.
-// ---------------------------------------------------------------------------------------------
-#ifndef LS_DIRECT
-#define LS_DIRECT 0
-#endif
-constexpr int kDirectWarps = 8;
-template <typename T, bool CLAMP, bool RESIDUAL, bool EMIT_T>
-__global__ void __launch_bounds__(kDirectWarps * 32)
-k_band_direct(const T* __restrict__ src, T* __restrict__ dst, Geom g, StencilParams<T> pr, TileArgs a) {
-    __shared__ uint32_t s_tm[kDirectWarps][64];
-    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const int count = *a.count;
-    T rmax = T(0);
-    int base = 0;
-    for (;;) {
-        if (lane == 0) base = (int)atomicAdd(a.ticket, (unsigned)kChunk);
-        base = __shfl_sync(0xffffffffu, base, 0);
-        if (base >= count) break;
-        for (int q = 0; q < kChunk && base + q < count; ++q) {
-            const QuadEntry e = a.qlist[a.reverse ? count - 1 - (base + q) : base + q];
-            const int quad = e.quad, nitems = e.nitems & 0xffff;
-            const int qx = quad % g.NQx, rest = quad / g.NQx, by = rest % g.NBy, bz = rest / g.NBy;
-            const int x0 = qx * 32, y0 = by * 8, z0 = bz * 8;
-            const bool edge = (qx == 0) | (by == 0) | (bz == 0) | (x0 + 33 > g.nx) | (y0 + 9 > g.ny) | (z0 + 9 > g.nz);
-            const uint16_t* items = a.items + (int64_t)quad * kItemsPerQuad;
-            if (EMIT_T) { s_tm[wib][lane] = 0u; s_tm[wib][lane + 32] = 0u; __syncwarp(); }
-            for (int p = lane; p < nitems; p += 32) {
-                const unsigned it = items[p];
-                const unsigned nib = it >> 9;
-                const int lz = (it >> 6) & 7, ly = (it >> 3) & 7, xq = it & 7;
-                const int x = x0 + xq * 4, y = y0 + ly, z = z0 + lz;
-                Item4<T> s;
-                auto ld4 = [&](int yy, int zz, T* o4) {
-                    const T* r = src + g.idx(x, yy, zz);
-                    if (sizeof(T) == 4) {
-                        const float4 v = __ldg(reinterpret_cast<const float4*>(r));
-                        o4[0] = (T)v.x; o4[1] = (T)v.y; o4[2] = (T)v.z; o4[3] = (T)v.w;
-                    } else {
-                        const double2 v0 = __ldg(reinterpret_cast<const double2*>(r)), v1 = __ldg(reinterpret_cast<const double2*>(r) + 1);
-                        o4[0] = (T)v0.x; o4[1] = (T)v0.y; o4[2] = (T)v1.x; o4[3] = (T)v1.y;
-                    }
-                };
-                if (!edge) {
-                    ld4(y, z, s.c); ld4(y - 1, z, s.ym); ld4(y + 1, z, s.yp); ld4(y, z - 1, s.zm); ld4(y, z + 1, s.zp);
-                    const T* r = src + g.idx(x, y, z);
-                    s.xm = __ldg(r - 1);
-                    s.xp = __ldg(r + 4);
-                } else {   // R3: edge replicate
-                    ld4(y, z, s.c); ld4(max(y - 1, 0), z, s.ym); ld4(min(y + 1, g.ny - 1), z, s.yp);
-                    ld4(y, max(z - 1, 0), s.zm); ld4(y, min(z + 1, g.nz - 1), s.zp);
-                    s.xm = __ldg(src + g.idx(max(x - 1, 0), y, z));
-                    s.xp = __ldg(src + g.idx(min(x + 4, g.nx - 1), y, z));
-                }
-                T v[4];
-                reinit_item<T>(s, pr, v);
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const bool on = (nib >> k) & 1u;
-                    if (RESIDUAL && on) rmax = fmax(rmax, mag(v[k] - s.c[k]));
-                    v[k] = on ? v[k] : s.c[k];
-                    if (CLAMP) v[k] = clamp_val(v[k], pr.gamma);
-                }
-                if (EMIT_T) {
-                    unsigned tn = 0;
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) tn |= (((nib >> k) & 1u) && mag(v[k]) < pr.gamma) ? (1u << k) : 0u;
-                    if (tn) atomicOr(&s_tm[wib][((xq >> 1) * 8 + lz) * 2 + (ly >> 2)], tn << ((ly & 3) * 8 + (xq & 1) * 4));
-                }
-                store4<T>(dst + g.idx(x, y, z), v);
-            }
-            if (EMIT_T) {
-                __syncwarp();
-                const uint64_t word = reinterpret_cast<const uint64_t*>(s_tm[wib])[lane];
-                a.tmask_out[(int64_t)quad * 32 + lane] = word;
-                const unsigned any = __ballot_sync(0xffffffffu, word != 0ull);
-                if (lane == 0) a.qflagT_out[quad] = any ? 1 : 0;
-                __syncwarp();
-            }
-        }
-    }
-    if (RESIDUAL) {
-        unsigned long long bits;
-        if (sizeof(T) == 4) bits = (unsigned long long)__float_as_uint((float)rmax);
-        else bits = (unsigned long long)__double_as_longlong((double)rmax);
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            const unsigned long long y = __shfl_xor_sync(0xffffffffu, bits, o);
-            bits = y > bits ? y : bits;
-        }
-        if (lane == 0 && bits != 0) atomicMax(a.residual, bits);
-    }
-    // self-resetting scheduler: the last warp to finish fetching zeroes the counters for the next launch
-    if (lane == 0) {
-        __threadfence();
-        if (atomicAdd(a.ticket + 1, 1u) == gridDim.x * kDirectWarps - 1) { a.ticket[0] = 0u; a.ticket[1] = 0u; }
-    }
-}
-
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -859,7 +768,10 @@ void launch_variant(const Maps& m, T* dst, const Geom& g, const StencilParams<T>
 #define LS_K1_NPW 0   // 0: one producer warp per stage
 #endif
     constexpr int NCW = K > 1 ? 8 : 4;
-    constexpr int STAGES = (K > 1 || ADV || sizeof(T) == 8) ? 2 : LS_K1_STAGES;
+#ifndef LS_ADV_STAGES
+#define LS_ADV_STAGES 2
+#endif
+    constexpr int STAGES = (K > 1 || sizeof(T) == 8) ? 2 : (ADV ? LS_ADV_STAGES : LS_K1_STAGES);
     // K = 1: gather warps (one per stage, or one for all stages); K = 2: one lane issuing TMA boxes
     constexpr int NPW = K > 1 ? 1 : (LS_K1_NPW ? LS_K1_NPW : STAGES);
     using S = Stage<T, K, ADV>;
@@ -887,11 +799,10 @@ bool launch_band_tile(const T* src, const T* F, T* dst, const Geom& g, const Ste
     if (K < 1 || K > 2 || (op.advance && K != 1)) return false;
     constexpr int XW = 16 / (int)sizeof(T);
     Maps m;
-    if (!make_map<T>(&m.M, src, g, 32, 8 + 2 * K, 8 + 2 * K)) return false;
-    if (!make_map<T>(&m.H, src, g, XW, 6 + 2 * K, 6 + 2 * K)) return false;
-    if (op.advance) {
-        if (!make_map<T>(&m.F, F, g, 32, 8, 8)) return false;
-    } else {
+    std::memset(&m, 0, sizeof m);
+    if (K == 2) {   // only the two-sweep kernels load whole boxes by TMA; the gather kernels take no tensor map
+        if (!make_map<T>(&m.M, src, g, 32, 8 + 2 * K, 8 + 2 * K)) return false;
+        if (!make_map<T>(&m.H, src, g, XW, 6 + 2 * K, 6 + 2 * K)) return false;
         m.F = m.M;
     }
     TileArgs a;
@@ -919,14 +830,7 @@ bool launch_band_tile(const T* src, const T* F, T* dst, const Geom& g, const Ste
         else if (op.clamp) launch_variant<T, false, KK, true, false, false>(m, dst, g, p, p, a, s);          \
         else launch_variant<T, false, KK, false, false, false>(m, dst, g, p, p, a, s);                       \
     } while (0)
-    if (LS_DIRECT && !op.advance && K == 1) {
-        static const int dgrid = [] { int n = 0; cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_band_direct<T, false, false, false>, kDirectWarps * 32, 0); return sm_count() * (n > 0 ? n : 1); }();
-        if (op.emit_T) k_band_direct<T, true, false, true><<<dgrid, kDirectWarps * 32, 0, s>>>(src, dst, g, p, a);
-        else if (op.residual && op.clamp) k_band_direct<T, true, true, false><<<dgrid, kDirectWarps * 32, 0, s>>>(src, dst, g, p, a);
-        else if (op.residual) k_band_direct<T, false, true, false><<<dgrid, kDirectWarps * 32, 0, s>>>(src, dst, g, p, a);
-        else if (op.clamp) k_band_direct<T, true, false, false><<<dgrid, kDirectWarps * 32, 0, s>>>(src, dst, g, p, a);
-        else k_band_direct<T, false, false, false><<<dgrid, kDirectWarps * 32, 0, s>>>(src, dst, g, p, a);
-    } else if (op.advance) launch_variant<T, true, 1, false, false, false>(m, dst, g, p, p, a, s);
+    if (op.advance) launch_variant<T, true, 1, false, false, false>(m, dst, g, p, p, a, s);
     else if (K == 2) LS_VARIANTS(2);
     else LS_VARIANTS(1);
 #undef LS_VARIANTS

@@ -706,3 +706,45 @@ def test_cfg5_runs_to_its_stopping_rule():
         assert np.array_equal(np.clip(one, -w.gamma, w.gamma)[inner][well], nxt[sl][inner][well])
         checked += int(well.sum())
     assert checked > 100000
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("shape", [(9, 13, 20), (17, 8, 33), (24, 40, 56)])
+def test_no_write_outside_the_fields(shape, dtype):
+    """compute-sanitizer is closed on the GPU pool, so out-of-bounds WRITES are looked for directly: phi, F and the
+    output field sit inside larger buffers whose guard zones (4096 elements before and after, a NaN pattern) must come
+    back untouched from every entry point, on the tile path and (nx % 4 != 0) on the scalar path, with bands that touch
+    the domain faces.  (Out-of-bounds reads would show as parity failures elsewhere: every result is compared bit for bit.)"""
+    G = 4096
+    dx = 1.0 / 32
+    phi, F = _random_band_field(shape, dtype, 91, dx)
+    F = (0.6 * F).astype(dtype)
+    n = phi.size
+    tdt = torch.float32 if dtype == np.float32 else torch.float64
+
+    def guarded(a):
+        buf = torch.full((n + 2 * G,), float("nan"), dtype=tdt, device="cuda")
+        view = buf[G:G + n].view(*shape)
+        if a is not None:
+            view.copy_(torch.from_numpy(a))
+        return buf, view
+
+    def intact(buf):
+        return bool(torch.isnan(buf[:G]).all().item() and torch.isnan(buf[G + n:]).all().item())
+
+    gamma, beta, dt, dtau = 4 * dx, 2 * dx, 0.4 * dx, 0.5 * dx
+    bp, vp = guarded(phi)
+    bF, vF = guarded(F)
+    bo, vo = guarded(None)
+    with Ctx(shape, dtype) as ctx:
+        ls.ls_build_band(ctx, vp, dx, gamma)
+        ls.ls_advance(ctx, vp, vF, dt, dx, beta, gamma, vo)
+        ls.ls_reinit(ctx, vo, vp, dtau, dx, gamma, 3)
+        ls.ls_reinit_tol(ctx, vo, vp, dtau, dx, gamma, 1e-3 * dx, 40, 5)
+        for fuse in (1, 2):
+            ls.ls_step(ctx, vp, vF, ls.make_params(dx, dt, dtau, beta, gamma, 5, ls.LS_REBUILD_INCREMENTAL, 0, fuse), 3)
+        ls.ls_step(ctx, vp, vF, ls.make_params(dx, dt, dtau, beta, gamma, 4, ls.LS_REBUILD_FULL, 0), 2)
+        ls.ls_advance(ctx, vp, vF, dt, dx, INF, INF, vo)
+        torch.cuda.synchronize()
+    assert intact(bp) and intact(bF) and intact(bo)
+    assert bool(torch.isfinite(vp).all().item()) and bool(torch.isfinite(vo).all().item())
