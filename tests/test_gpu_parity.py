@@ -748,3 +748,31 @@ def test_no_write_outside_the_fields(shape, dtype):
         torch.cuda.synchronize()
     assert intact(bp) and intact(bF) and intact(bo)
     assert bool(torch.isfinite(vp).all().item()) and bool(torch.isfinite(vo).all().item())
+
+
+@pytest.mark.parametrize("iters", [5, 4])
+@pytest.mark.parametrize("shape", [(24, 40, 56), (17, 8, 33)])
+def test_advance_and_export_after_incremental_step(shape, iters):
+    """ls.h: ls_advance and ls_band_export use 'the band last built', and the last step of ls_step counts as a build
+    (the band of phi^{n-1}).  With LS_REBUILD_INCREMENTAL the launch that writes phi^n also emits the T masks of phi^n
+    for the NEXT step; they go into the other half of a double buffer and must not be what ls_advance / ls_band_export
+    see (round-1 advisor finding: they did).  Odd and even `iters` (last sweep / band copy emits), tile and scalar path."""
+    dx = 1.0 / 32
+    phi, F = _random_band_field(shape, np.float32, 55, dx)
+    F = (0.6 * F).astype(np.float32)
+    gamma, beta, dt, dtau = 4 * dx, 2 * dx, 0.4 * dx, 0.5 * dx
+    phi1, _ = orc.step(phi, F, dx, dt, dtau, beta, gamma, iters, 1)
+    phi2, _ = orc.step(phi1, F, dx, dt, dtau, beta, gamma, iters, 1)
+    Tm1, _ = orc.band_masks(phi1, gamma)                      # the band the second step built
+    want = orc.advance(phi2, F, Tm1, dt, dx, beta, gamma)     # eq. 8 on THAT T, applied to the current field
+    with Ctx(shape, np.float32) as ctx:
+        d_phi, d_F = to_dev(phi), to_dev(F)
+        ls.ls_step(ctx, d_phi, d_F, ls.make_params(dx, dt, dtau, beta, gamma, iters, ls.LS_REBUILD_INCREMENTAL), 2)
+        assert np.array_equal(d_phi.cpu().numpy(), phi2)
+        assert_band_equal(ctx, phi1, gamma)
+        out = torch.empty_like(d_phi)
+        ls.ls_advance(ctx, d_phi, d_F, dt, dx, beta, gamma, out)
+        got = out.cpu().numpy()
+        assert_band_equal(ctx, phi1, gamma)                  # still the band last built
+    assert np.array_equal(got, want)
+    assert (Tm1 != orc.band_masks(phi2, gamma)[0]).any()      # the two bands do differ: the test can tell them apart
