@@ -33,13 +33,18 @@ def nvcc_path() -> str:
 
 
 def source_sha() -> str:
-    """Hash of the kernel sources (csrc/ and include/ls.h): ties an ncu capture summary to the code it measured."""
+    """Hash of the kernel CODE (csrc/ and include/ls.h with comments and white space removed): ties an ncu capture
+    summary to the code it measured, and survives edits of comments."""
     import hashlib
+    import re
     h = hashlib.sha256()
     for f in sorted(CSRC.iterdir()) + [PKG.parent / "include" / "ls.h"]:
         if f.suffix in (".cu", ".cuh", ".h"):
+            text = f.read_text()
+            text = re.sub(r"/\*.*?\*/", " ", text, flags=re.S)      # block comments
+            text = re.sub(r"//[^\n]*", " ", text)                    # line comments (no string literal here holds "//")
             h.update(f.name.encode())
-            h.update(f.read_bytes())
+            h.update(" ".join(text.split()).encode())
     return h.hexdigest()[:16]
 
 

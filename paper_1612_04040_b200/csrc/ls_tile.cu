@@ -1,24 +1,26 @@
-// ls_tile.cu — the band kernels of Steps 2 and 3: persistent, warp-specialised, TMA-fed.
+// ls_tile.cu — the band kernels of Steps 2 and 3: persistent, warp-specialised, fed by asynchronous
+// copies through an mbarrier pipeline.
 //
 // Tile = one QUAD (four x-adjacent 8^3 bricks, 32 x 8 x 8 points; ls_internal.h).  In shared memory:
 //   M  [8+2K][8+2K][32]   the quad and K halo rows in y and z: every row is one aligned 128-byte line (fp32)
-//   L, R [6+2K][6+2K][XW] the x halo, one 16-byte piece per row (fp32: 4 cells, fp64: 2), loaded only when an
-//                         N point sits on that edge of the quad (K = 1) — a third of the sectors otherwise
-// K = number of operations fused in the launch: K = 1 is Advance or one reinit sweep; K = 2 is two sweeps
-// (temporal blocking of eq. 12's pseudo-time iterations): sweep 1 is evaluated on the
+//   L, R [6+2K][6+2K][XW] the x halo, one 16-byte piece per row (fp32: 4 cells, fp64: 2)
+// K = number of operations fused in the launch: K = 1 is Advance or one reinit sweep (the default); K = 2 is two
+// sweeps (temporal blocking of eq. 12's pseudo-time iterations): sweep 1 is evaluated on the
 // quad's N points AND on the N points of the one-cell ring around it (neighbour quads' masks), kept in
 // registers until every read of iteration k is done, written back IN PLACE, and sweep 2 then runs on the
 // quad's own points.  Jacobi order is preserved exactly, so K = 2 equals two K = 1 launches bit for bit.
 //
-//   producer warp (one elected lane)   takes quads from the ordered quad list through a device ticket
-//        counter (chunks of 4), and per quad issues up to three cp.async.bulk.tensor.3d box loads (M, L, R)
-//        straight from the dense x-fastest field, one cp.async.bulk of the quad's
-//        precomputed item list (Advance: the 32x8x8 box of F and the quad's 32 T mask words; K = 2: the N
-//        masks of the six neighbour quads), all completing on the stage's "full" mbarrier; it waits on the
-//        stage's "empty" mbarrier before reuse.
-//   consumer warps   wait on "full"; edge-replicate the out-of-domain halo (R3; TMA zero-fills it); lane l
-//        evaluates items l, l+NC, ...: one item = 4 x-consecutive cells = 5 LDS.128 + 2 LDS.32, two packed
-//        fp32 pairs through eq. 3-8 / eq. 12-13 (ls_math.cuh), one 16-byte store to the other global buffer.
+//   producer warps, K = 1 (one whole warp per pipeline stage)   draw one quad at a time from the ordered quad list
+//        through a device ticket counter, read its list entry and load map, and GATHER only the 32-byte sectors
+//        the quad's N points read with 16-byte cp.async (LDGSTS), two lanes per sector (half the DRAM reads of a
+//        whole-box load); the quad's precomputed item list comes by cp.async.bulk (UBLKCP); Advance also gathers
+//        the F rows of bricks that hold band points and takes the quad's 32 T mask words by cp.async.bulk.
+//   producer, K = 2 (one elected lane)   issues three cp.async.bulk.tensor.3d box loads (M, L, R: UTMALDG) straight
+//        from the dense x-fastest field, the item list and the N masks of the six neighbour quads.
+//        Either way everything completes on the stage's "full" mbarrier, and the stage's "empty" mbarrier gates its reuse.
+//   consumer warps   wait on "full"; edge-replicate the out-of-domain halo of tiles that reach outside the domain
+//        (R3); lane l evaluates items l, l+NC, ...: one item = 4 x-consecutive cells = 5 LDS.128 + 2 LDS.32, two
+//        packed fp32 pairs through eq. 3-8 / eq. 12-13 (ls_math.cuh), one 16-byte store to the other global buffer.
 //        K = 1 needs no CTA barrier per tile: each warp arrives on "empty" when it is done with the stage.
 // The arithmetic is bit-identical to the scalar kernels of ls_stencil.cu, which remain the path for grids the
 // tile path cannot address (nx not a multiple of 4, unaligned fields).
