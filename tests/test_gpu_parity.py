@@ -578,12 +578,14 @@ def test_step_snapshots_match_oracle_trajectory():
 # from the GPU's own phi^{N-1} crops.  The incremental rebuild's exactness argument (T^{n+1} inside N^n)
 # is the kind of thing that breaks late (fronts merging in cfg 3, the band reaching the domain faces), not at step 3.
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("cfg,total", [(4, 200), (3, 100)])
-def test_full_size_late_step_windowed(cfg, total):
+@pytest.mark.parametrize("cfg,total,rebuild", [(4, 200, ls.LS_REBUILD_INCREMENTAL), (4, 77, ls.LS_REBUILD_INCREMENTAL),
+                                               (3, 100, ls.LS_REBUILD_INCREMENTAL),
+                                               (3, 100, ls.LS_REBUILD_FULL)])
+def test_full_size_late_step_windowed(cfg, total, rebuild):
     w = inputs.config(cfg)
     n, size, margin = w.nx, 112, 8
-    p0 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, ls.LS_REBUILD_INCREMENTAL, 0)
-    p1 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, ls.LS_REBUILD_INCREMENTAL, 1)
+    p0 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild, 0)
+    p1 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild, 1)
     with Ctx(w.shape, w.dtype) as ctx:
         d_phi, d_F = to_dev(w.phi), to_dev(w.F)
         ls.ls_step(ctx, d_phi, d_F, p0, 1)
