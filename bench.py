@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — throughput of the narrow-band level-set hot path on B200 (contract: task prompt).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1..5] [--n EDGE]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1..5] [--edge EDGE]
                     [--rebuild incremental|full] [--fuse 0|1|2]
 
 Workload: BASELINE.json configs[--config - 1]; default 4 (cfg 4: 1024^3 fp32 torus, the config north_star quotes its
@@ -81,7 +81,8 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config 1..5 (1-based); the bench line is 4; 2 = dense advance, 5 = fp64 reinit sweeps")
-    ap.add_argument("--n", type=int, default=None, help="grid edge override (smoke runs of the bench itself)")
+    ap.add_argument("--edge", "--n", dest="n", type=int, default=None,
+                    help="grid edge override (smaller or paper-shaped grids; under torchrun spell it --edge: its own parser claims --n)")
     ap.add_argument("--rebuild", default="incremental", choices=["incremental", "full"])
     ap.add_argument("--fuse", type=int, default=0, choices=[0, 1, 2],
                     help="reinit sweeps per launch: 0 = library default (1), 1 = one sweep per launch, 2 = temporal blocking")
