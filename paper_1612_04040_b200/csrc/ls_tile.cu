@@ -769,11 +769,19 @@ void launch_variant(const Maps& m, T* dst, const Geom& g, const StencilParams<T>
 #ifndef LS_K1_NPW
 #define LS_K1_NPW 0   // 0: one producer warp per stage
 #endif
-    constexpr int NCW = K > 1 ? 8 : 4;
+#ifndef LS_F64_NCW
+#define LS_F64_NCW 8
+#endif
+#ifndef LS_F64_STAGES
+#define LS_F64_STAGES 2
+#endif
+    // consumer warps per CTA: four is the measured optimum in fp32; fp64 needs 80 registers and 29 KB
+    // per stage, so few CTAs fit an SM and eight consumer warps each keep more of them in flight (78.7 against 82.5 us)
+    constexpr int NCW = K > 1 ? 8 : (sizeof(T) == 8 ? LS_F64_NCW : 4);
 #ifndef LS_ADV_STAGES
 #define LS_ADV_STAGES 2
 #endif
-    constexpr int STAGES = (K > 1 || sizeof(T) == 8) ? 2 : (ADV ? LS_ADV_STAGES : LS_K1_STAGES);
+    constexpr int STAGES = K > 1 ? 2 : (sizeof(T) == 8 ? LS_F64_STAGES : (ADV ? LS_ADV_STAGES : LS_K1_STAGES));
     // K = 1: gather warps (one per stage, or one for all stages); K = 2: one lane issuing TMA boxes
     constexpr int NPW = K > 1 ? 1 : (LS_K1_NPW ? LS_K1_NPW : STAGES);
     using S = Stage<T, K, ADV>;
