@@ -778,3 +778,36 @@ def test_advance_and_export_after_incremental_step(shape, iters):
         assert_band_equal(ctx, phi1, gamma)                  # still the band last built
     assert np.array_equal(got, want)
     assert (Tm1 != orc.band_masks(phi2, gamma)[0]).any()      # the two bands do differ: the test can tell them apart
+
+
+@pytest.mark.parametrize("seed", list(range(int(__import__("os").environ.get("LS_FUZZ", "12")))))
+def test_random_shapes_and_parameters(seed):
+    """Seeded random cases: shape (ragged; nx a multiple of 4 or not: tile or scalar path), dtype, gamma / beta / dt / dtau,
+    iters (odd, even, 0), rebuild mode, sweeps per launch, chunking of the steps into chained calls — free running for a
+    few steps, band export and field compared with the oracle bit for bit."""
+    u = inputs.uniform01(7000 + seed, 0, 16)
+    dtype = np.float32 if u[0] < 0.6 else np.float64
+    nx = int(4 + u[1] * 70); nx = nx - nx % 4 if u[2] < 0.7 else nx | 1
+    shape = (int(3 + u[3] * 40), int(3 + u[4] * 40), max(nx, 4))
+    dx = 1.0 / 32
+    gamma = (2.0 + 5.0 * u[5]) * dx
+    beta = gamma * (0.3 + 0.5 * u[6])
+    dt, dtau = (0.2 + 0.3 * u[7]) * dx, (0.2 + 0.3 * u[8]) * dx
+    iters = int(u[9] * 7)
+    rebuild = ls.LS_REBUILD_INCREMENTAL if u[10] < 0.6 else ls.LS_REBUILD_FULL
+    fuse = 2 if u[11] < 0.4 else 1
+    steps = 2 + int(u[12] * 4)
+    first = 1 + int(u[13] * (steps - 1))
+    phi, F = _random_band_field(shape, dtype, 7100 + seed, dx)
+    F = (0.8 * F).astype(dtype)
+    want, upd = orc.step(phi, F, dx, dt, dtau, beta, gamma, iters, steps)
+    prev, _ = orc.step(phi, F, dx, dt, dtau, beta, gamma, iters, steps - 1)
+    with Ctx(shape, dtype) as ctx:
+        d_phi, d_F = to_dev(phi), to_dev(F)
+        ls.ls_step(ctx, d_phi, d_F, ls.make_params(dx, dt, dtau, beta, gamma, iters, rebuild, 0, fuse), first)
+        if steps > first:
+            ls.ls_step(ctx, d_phi, d_F, ls.make_params(dx, dt, dtau, beta, gamma, iters, rebuild, 1, fuse), steps - first)
+        got = d_phi.cpu().numpy()
+        assert ls.ls_stats(ctx)[0] == upd
+        assert_band_equal(ctx, prev, gamma)
+    assert np.array_equal(got, want), (shape, dtype, iters, rebuild, fuse, max_err_dx(got, want, dx))
