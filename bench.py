@@ -394,7 +394,9 @@ def report(args, w, out, world, K, W, esz):
         traffic = (float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])) if row else None
         r = {"bound": "hbm", "kernel": what, "achieved": ach, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
              "frac": ach / peak, "traffic": traffic, "traffic_source": ncu_note if row else None,
-             "algorithmic_bytes_per_launch": alg_bytes, "us_per_launch": us, "frac_of_8TBps_nominal": ach / 8000.0}
+             "algorithmic_bytes_per_launch": alg_bytes, "us_per_launch": us, "frac_of_8TBps_nominal": ach / 8000.0,
+             "overfetch": (traffic / alg_bytes) if traffic else None,
+             "dram_gbs": (traffic / (us * 1e-6) * 1e-9) if traffic else None}
         if row:   # issue-slot view of the same launch (the band kernels are bound by instruction issue)
             alu_peak = ISSUE_SLOTS_PER_CLOCK * sm_mhz * 1e6 * 1e-12
             alu_ach = float(row["warp_instructions"]) / (us * 1e-6) * 1e-12
@@ -442,6 +444,8 @@ def report(args, w, out, world, K, W, esz):
         "roofline": roofline, "roofline_advance": roofline_advance, "full_rebuild": out.get("full_rebuild"),
         "kernels": kernels, "cpu_baseline": cpu,
     }
+    if w.mode == "band" and "band" in kernels:   # the whole-step figure with the build included and excluded
+        line["ms_per_step_without_band_build"] = out["ms"] / K - kernels["band"]["ms_per_step"]
     print(json.dumps(line), flush=True)
 
 
