@@ -53,8 +53,8 @@ struct ScalarArgs {
     unsigned long long* residual;
 };
 
-// Scalar band kernel for grids the tile path cannot address: one CTA per listed quad and turn, one thread per
-// cell of a brick layer pair, brick by brick.  Same arithmetic (scalar functions of ls_math.cuh), same writes:
+// Scalar band kernel for grids the tile path cannot address: one CTA per brick of a listed quad and turn, one thread
+// per cell of a brick layer pair.  Same arithmetic (scalar functions of ls_math.cuh), same writes:
 // every N cell of the quad gets the new value (kAdvance: N cells outside T are copied).
 template <typename T, int MODE, bool CLAMP, bool RESIDUAL, bool EMIT_T>
 __global__ void __launch_bounds__(kBandThreads) k_band_scalar(const T* __restrict__ src, const T* __restrict__ F,
@@ -62,17 +62,20 @@ __global__ void __launch_bounds__(kBandThreads) k_band_scalar(const T* __restric
                                                               ScalarArgs a) {
     __shared__ T s[kTileElems];
     __shared__ uint32_t halves[8][2];
-    __shared__ int s_any;
     const int count = *a.count;
     const int lx = threadIdx.x & 7, ly = (threadIdx.x >> 3) & 7, lz0 = threadIdx.x >> 6;
     T rmax = T(0);
-    for (int li = blockIdx.x; li < count; li += gridDim.x) {
-        const int quad = a.qlist[li].quad;
+    // Work unit = one brick of a listed quad (4 per list entry): the grids this path serves are small or oddly shaped,
+    // and a CTA that walked the four bricks of a quad one after the other made a launch four tile-load latencies long.
+    for (int wi = blockIdx.x; wi < count * 4; wi += gridDim.x) {
+        const int quad = a.qlist[wi >> 2].quad, j = wi & 3;
         const int qx = quad % g.NQx, rest = quad / g.NQx, by = rest % g.NBy, bz = rest / g.NBy;
         bool tvalid = false;
         if (MODE == kAdvance) tvalid = a.qflagT_in[quad] != 0 && (a.tgate == nullptr || a.tgate[quad] != 0);
-        if (EMIT_T && threadIdx.x == 0) s_any = 0;
-        for (int j = 0; j < 4; ++j) {
+        // EMIT_T: the quad's flag only says "the T masks may hold a bit" (they are all written, zeros included), so
+        // the bricks of a quad need not agree on it across CTAs
+        if (EMIT_T && j == 0 && threadIdx.x == 0) a.qflagT_out[quad] = 1;
+        {
             const int bx = qx * 4 + j;
             const uint64_t* nw = a.nmask + (int64_t)quad * 32 + j * 8;
             uint64_t any = 0;
@@ -123,14 +126,8 @@ __global__ void __launch_bounds__(kBandThreads) k_band_scalar(const T* __restric
                 if (threadIdx.x < 8) {
                     const uint64_t word = (uint64_t)halves[threadIdx.x][0] | ((uint64_t)halves[threadIdx.x][1] << 32);
                     a.tmask_out[(int64_t)quad * 32 + j * 8 + threadIdx.x] = word;
-                    if (word) s_any = 1;
                 }
             }
-        }
-        if (EMIT_T) {
-            __syncthreads();
-            if (threadIdx.x == 0) a.qflagT_out[quad] = s_any ? 1 : 0;
-            __syncthreads();
         }
     }
     if (RESIDUAL) {
