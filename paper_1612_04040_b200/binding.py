@@ -28,6 +28,9 @@ SYMBOLS = (
     "ls_band_export", "ls_advance", "ls_reinit", "ls_reinit_tol", "ls_step", "ls_step_host", "ls_stats",
     "ls_stats_reset", "ls_profile_enable", "ls_profile_read", "ls_profile_reset", "ls_selftest_math", "ls_step_snapshots",
 )
+# every symbol include/ls_static.h declares (tests/test_zz_no_alloc.py checks them)
+STATIC_SYMBOLS = ("ls_tube_static_setup", "ls_tube_static", "ls_tube_static_error")
+LS_TUBE_STATIC_MAX_BRICKS = 65536
 
 
 class ls_params(C.Structure):
@@ -80,6 +83,12 @@ def lib() -> C.CDLL:
         L.ls_selftest_math.argtypes = [_P, C.c_uint64, _L, _D, _D, _D, _D, C.POINTER(_L)]
         for name in SYMBOLS[2:]:
             getattr(L, name).restype = C.c_int
+        L.ls_tube_static_setup.argtypes = []
+        L.ls_tube_static_setup.restype = C.c_int
+        L.ls_tube_static.argtypes = [_P, _I, _I, _I, C.c_int, _D, _P, _P, _P, _P]
+        L.ls_tube_static.restype = C.c_int
+        L.ls_tube_static_error.argtypes = []
+        L.ls_tube_static_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -218,3 +227,18 @@ def ls_step_snapshots(ctx: int, phi, F, p: ls_params, n_steps: int, every: int, 
                                 _P(_host(host_out)) if host_out is not None else None, C.byref(n)),
         "ls_step_snapshots")
     return n.value
+
+
+def ls_tube_static_setup() -> None:
+    st = lib().ls_tube_static_setup()
+    if st != LS_OK:
+        raise LsError(st, "ls_tube_static_setup: " + lib().ls_tube_static_error().decode())
+
+
+def ls_tube_static(phi, nx: int, ny: int, nz: int, dtype: int, gamma: float, cuda_stream: int, T_ids, T_masks, counts) -> None:
+    """include/ls_static.h: T tube with no ctx and no allocation.  T_ids int32[nbricks], T_masks int64/uint64[8*nbricks],
+    counts int64[2] are DEVICE tensors (or addresses) the caller owns; nothing is read back here."""
+    st = lib().ls_tube_static(_P(_dev(phi)), nx, ny, nz, dtype, gamma, _P(cuda_stream), _P(_dev(T_ids)), _P(_dev(T_masks)),
+                              _P(_dev(counts)))
+    if st != LS_OK:
+        raise LsError(st, "ls_tube_static: " + lib().ls_tube_static_error().decode())

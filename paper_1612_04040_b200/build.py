@@ -18,7 +18,10 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 SO = PKG / "libls.so"
-SOURCES = ["ls_band.cu", "ls_stencil.cu", "ls_tile.cu", "ls_api.cu"]
+SOURCES = ["ls_band.cu", "ls_stencil.cu", "ls_tile.cu", "ls_api.cu", "ls_static.cu"]
+# ls_static.cu (include/ls_static.h: the entry point that allocates nothing) is a translation unit of its own that shares no
+# code with the others; source_sha() leaves it out, so the hash names the code of the ls.h path that profiles/ measured.
+UNHASHED = {"ls_static.cu"}
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-fmad=false",
     "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math,-Wall", "-cudart", "static", "-shared",
@@ -39,7 +42,7 @@ def source_sha() -> str:
     import re
     h = hashlib.sha256()
     for f in sorted(CSRC.iterdir()) + [PKG.parent / "include" / "ls.h"]:
-        if f.suffix in (".cu", ".cuh", ".h"):
+        if f.suffix in (".cu", ".cuh", ".h") and f.name not in UNHASHED:
             text = f.read_text()
             text = re.sub(r"/\*.*?\*/", " ", text, flags=re.S)      # block comments
             text = re.sub(r"//[^\n]*", " ", text)                    # line comments (no string literal here holds "//")
@@ -52,7 +55,8 @@ def needs_build() -> bool:
     if not SO.exists():
         return True
     t = SO.stat().st_mtime
-    deps = [CSRC / s for s in SOURCES] + [CSRC / "ls_internal.h", CSRC / "ls_math.cuh", PKG.parent / "include" / "ls.h", Path(__file__)]
+    deps = [CSRC / s for s in SOURCES] + [CSRC / "ls_internal.h", CSRC / "ls_math.cuh", PKG.parent / "include" / "ls.h",
+                                          PKG.parent / "include" / "ls_static.h", Path(__file__)]
     return any(d.stat().st_mtime > t for d in deps)
 
 
