@@ -355,7 +355,8 @@ def run_ours(args):
                             "d2h_bytes_per_step": w.n_points * esz, "steps": Ke, "ms_per_step": dt / Ke * 1e3,
                             "pcie_gbs": 2 * w.n_points * esz * Ke / dt * 1e-9,
                             "call": "ls_step_host(n_steps=1) per step: pinned host phi in, phi out; the static F was uploaded "
-                                    "once by the warm-up call (F_host = NULL afterwards)"})
+                                    "once by the warm-up call (F_host = NULL afterwards); fields >= 64 MiB go through the "
+                                    "library's z-slab pipeline (H2D / kernels / D2H overlapped, every layer copied once each way)"})
             del hp
     finally:
         ls.ls_destroy(ctx)

@@ -160,7 +160,15 @@ ls_status ls_step(ls_ctx* ctx, void* phi, const void* F, const ls_params* p, int
 /* Same as ls_step with HOST buffers (pageable or pinned): copies phi and F to ctx-owned device
  * fields, runs n_steps, copies phi back, and synchronises.  The end-to-end entry point.
  * F is static (R17): F_host = NULL reuses the F that the last call with a non-NULL F_host left on the
- * device (LS_ERR_STATE if there was none), which saves a third of the transfer. */
+ * device (LS_ERR_STATE if there was none), which saves a third of the transfer.
+ * A call with n_steps == 1 on a field of at least 64 MiB runs as a pipeline of z-slabs: one step depends on
+ * p->iters + 1 layers around a point (eq. 3-5, 11, 12), so each slab is stepped on a window with that many halo
+ * layers (ctx-owned window buffers and a child ctx of the window's shape) while later slabs are still being
+ * uploaded and earlier ones downloaded — host-to-device copy, kernels and device-to-host copy overlap on three
+ * ctx-owned streams (pinned host memory makes the copies asynchronous; pageable works).  The result and the work
+ * counters (ls_stats) are bit-identical to the unsliced call; after such a call the ctx holds no band
+ * (ls_band_counts / ls_band_export / ls_advance return LS_ERR_STATE until the next build), and ls_profile_* does
+ * not see the windows' kernels. */
 ls_status ls_step_host(ls_ctx* ctx, void* phi_host, const void* F_host, const ls_params* p, int32_t n_steps);
 
 /* m-step batching with snapshot return (the paper keeps m results on the device and

@@ -1,6 +1,7 @@
 // ls_api.cu — the C ABI of include/ls.h: context, argument checks, and the host driver of the
 // Step 1-3 loop on one stream.  Every step of the path runs in the kernels of
 // ls_band.cu / ls_tile.cu / ls_stencil.cu; this file only sequences launches.  There is no CPU fallback.
+#include <algorithm>
 #include <cmath>
 #include <cstddef>
 #include <cstdio>
@@ -13,6 +14,8 @@
 #include "../../include/ls.h"
 #include "ls_internal.h"
 
+struct HostPipe;
+
 struct ls_ctx {
     ls::Geom g;
     ls_dtype dtype;
@@ -22,6 +25,7 @@ struct ls_ctx {
     void* dev_phi;        // ls_step_host staging (lazy)
     void* dev_F;
     bool dev_F_valid;     // dev_F holds the F of the last ls_step_host call that passed one
+    struct HostPipe* pipe;   // ls_step_host: the z-slab pipeline of one-step calls on large grids (lazy)
     void* snap[2];        // ls_step_snapshots: device snapshot slots (lazy)
     cudaStream_t copy_stream;   // ... and the stream / events of the device-to-host copies (lazy)
     cudaEvent_t snap_ready[2], snap_free[2];
@@ -278,6 +282,165 @@ ls_status check_step_args(ls_ctx* c, const void* phi, const void* F, const ls_pa
 
 }  // namespace
 
+// ---- ls_step_host, one step per call on a large grid: z-slab pipeline ---------------------------------------------
+// A one-step call moves the whole field host -> device -> host (2 x 4.3 GB at cfg 4: ~78 ms each way) around ~5 ms of
+// GPU work; on one stream the three phases run one after the other.  One narrow-band step has a finite domain of
+// dependence: Advance reads the face neighbours of a point, each of the `iters` Jacobi sweeps one more layer, the T / N
+// membership one layer, eq. 10 none (eq. 3-5, 11, 12) — phi^{n+1} on the layers [z0, z1) is a
+// function of phi^n on [z0 - h, z1 + h), h = iters + 1.  So the field is cut into z-slabs (the paper's own decomposition
+// axis is a slab cut too): slab k's layers are uploaded ONCE into the full staging field, the step runs on
+// a window of the staging field that holds the slab plus h layers on each side (copied device-to-device into a window
+// buffer: the staging field must stay phi^n for the neighbouring windows), on a child ctx of the window's shape, and the
+// slab's layers of the result go back to the host while later slabs are still arriving: H2D, compute and D2H overlap on
+// three streams.  The window's z ends are the child's domain boundary (edge replicate, R3): exact where they are the
+// grid's own boundary, wrong within iters layers of an artificial cut — layers that are never returned.  Results are
+// bit-identical to the unsliced call; every window has the same shape (the first and last are shifted inwards).
+struct HostPipe {
+    ls_ctx* child;
+    int L, zs, h;                 // window layers, slab layers, halo layers
+    void* buf[3];                 // window fields
+    cudaStream_t up, cs, down;
+    cudaEvent_t start, done[3], freed[3];
+    std::vector<cudaEvent_t>* uploaded;   // one per slab
+};
+
+namespace {
+
+void pipe_destroy(HostPipe* hp) {
+    if (!hp) return;
+    if (hp->child) ls_destroy(hp->child);
+    for (void* b : hp->buf)
+        if (b) cudaFree(b);
+    if (hp->up) cudaStreamDestroy(hp->up);
+    if (hp->cs) cudaStreamDestroy(hp->cs);
+    if (hp->down) cudaStreamDestroy(hp->down);
+    if (hp->start) cudaEventDestroy(hp->start);
+    for (int i = 0; i < 3; ++i) {
+        if (hp->done[i]) cudaEventDestroy(hp->done[i]);
+        if (hp->freed[i]) cudaEventDestroy(hp->freed[i]);
+    }
+    if (hp->uploaded) {
+        for (cudaEvent_t e : *hp->uploaded) cudaEventDestroy(e);
+        delete hp->uploaded;
+    }
+    cudaGetLastError();
+    delete hp;
+}
+
+// Slab thickness for a one-step call, or 0 when the call should run unsliced (small field, few layers, not one step).
+int pipe_slab_layers(const ls_ctx* c, const ls_params* p, int n_steps) {
+    if (n_steps != 1) return 0;
+    const size_t plane = (size_t)c->g.nx * c->g.ny * c->elem;
+    if (plane * (size_t)c->g.nz < ((size_t)64 << 20)) return 0;        // transfers too short to be worth the windows
+    const int64_t h = (int64_t)p->iters + 1;
+    int64_t zs = (int64_t)((((size_t)16 << 20) + plane - 1) / plane);   // >= 16 MiB per slab
+    if (zs < 4 * h) zs = 4 * h;                                        // <= 1.5 x redundant compute
+    if (zs < 8) zs = 8;
+    if (zs + 2 * h > c->g.nz || 2 * zs > c->g.nz) return 0;            // window must fit; at least two slabs
+    return (int)zs;
+}
+
+ls_status pipe_ensure(ls_ctx* c, int zs, int h) {
+    const int L = zs + 2 * h;
+    if (c->pipe && c->pipe->L == L && c->pipe->zs == zs) return LS_OK;
+    pipe_destroy(c->pipe);
+    c->pipe = nullptr;
+    HostPipe* hp = new (std::nothrow) HostPipe();
+    if (!hp) return LS_ERR_ALLOC;
+    std::memset(hp, 0, sizeof *hp);
+    hp->L = L; hp->zs = zs; hp->h = h;
+    hp->uploaded = new (std::nothrow) std::vector<cudaEvent_t>();
+    cudaError_t e = hp->uploaded ? cudaSuccess : cudaErrorMemoryAllocation;
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&hp->up, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&hp->cs, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&hp->down, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&hp->start, cudaEventDisableTiming);
+    for (int i = 0; i < 3 && e == cudaSuccess; ++i) {
+        e = cudaEventCreateWithFlags(&hp->done[i], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&hp->freed[i], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaMalloc(&hp->buf[i], (size_t)c->g.nx * c->g.ny * L * c->elem);
+    }
+    const int K = (c->g.nz + zs - 1) / zs;
+    for (int k = 0; k < K && e == cudaSuccess; ++k) {
+        cudaEvent_t ev;
+        e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+        if (e == cudaSuccess) hp->uploaded->push_back(ev);
+    }
+    ls_status st = LS_OK;
+    if (e != cudaSuccess) {
+        st = e == cudaErrorMemoryAllocation ? LS_ERR_ALLOC : cuda_fail(e, "ls_step_host: slab pipeline set-up");
+        cudaGetLastError();
+    } else {
+        st = ls_create(c->g.nx, c->g.ny, L, c->dtype, (void*)hp->cs, &hp->child);
+    }
+    if (st != LS_OK) { pipe_destroy(hp); return st; }
+    c->pipe = hp;
+    return LS_OK;
+}
+
+// The sliced one-step call.  c->dev_phi / c->dev_F are allocated, F is on the device (this call's upload, if any, is queued
+// on c->stream).  Synchronises; on a failure it still drains its streams before it returns the first error.
+ls_status step_host_sliced(ls_ctx* c, void* phi_host, const ls_params* p, int zs) {
+    const int h = p->iters + 1;
+    ls_status st = pipe_ensure(c, zs, h);
+    if (st != LS_OK) return st;
+    HostPipe* hp = c->pipe;
+    ls_ctx* ch = hp->child;
+    const int nz = c->g.nz, L = hp->L, K = (nz + zs - 1) / zs;
+    const size_t plane = (size_t)c->g.nx * c->g.ny * c->elem;
+    ls_params q = *p;
+    q.chained = 0;
+    cudaError_t ce = cudaSuccess;
+    const char* what = "";
+    auto ck = [&](cudaError_t e, const char* w) { if (ce == cudaSuccess && e != cudaSuccess) { ce = e; what = w; } return e == cudaSuccess; };
+    const int64_t child_launches0 = ch->launches;
+    int64_t extra_launches = 0;
+    bool ok = ck(cudaEventRecord(hp->start, c->stream), "cudaEventRecord") &&
+              ck(cudaStreamWaitEvent(hp->up, hp->start, 0), "cudaStreamWaitEvent") &&
+              ck(cudaStreamWaitEvent(hp->cs, hp->start, 0), "cudaStreamWaitEvent") &&
+              ck(cudaStreamWaitEvent(hp->down, hp->start, 0), "cudaStreamWaitEvent");
+    // every layer goes up once, slab by slab
+    for (int k = 0; k < K && ok; ++k) {
+        const int z0 = k * zs, z1 = std::min(nz, z0 + zs);
+        ok = ck(cudaMemcpyAsync((char*)c->dev_phi + z0 * plane, (const char*)phi_host + z0 * plane, (z1 - z0) * plane,
+                                cudaMemcpyHostToDevice, hp->up), "slab upload") &&
+             ck(cudaEventRecord((*hp->uploaded)[k], hp->up), "cudaEventRecord");
+    }
+    for (int k = 0; k < K && ok && st == LS_OK; ++k) {
+        const int z0 = k * zs, z1 = std::min(nz, z0 + zs), b = k % 3;
+        const int lo = std::max(0, std::min(z0 - h, nz - L));       // window [lo, lo + L): same shape for every slab
+        const int last_slab = (lo + L - 1) / zs;                    // uploads are ordered: the last slab it touches
+        ok = ck(cudaStreamWaitEvent(hp->cs, (*hp->uploaded)[last_slab], 0), "cudaStreamWaitEvent");
+        if (ok && k >= 3) ok = ck(cudaStreamWaitEvent(hp->cs, hp->freed[b], 0), "cudaStreamWaitEvent");   // its download has drained
+        if (!ok) break;
+        ok = ck(cudaMemcpyAsync(hp->buf[b], (const char*)c->dev_phi + lo * plane, L * plane, cudaMemcpyDeviceToDevice, hp->cs),
+                "window copy");
+        if (!ok) break;
+        const void* Fwin = (const char*)c->dev_F + lo * plane;
+        st = c->dtype == LS_F32 ? step_impl<float>(ch, (float*)hp->buf[b], (const float*)Fwin, &q, 1)
+                                : step_impl<double>(ch, (double*)hp->buf[b], (const double*)Fwin, &q, 1);
+        if (st != LS_OK) break;
+        // work counters of the parent: each grid point once (the window's halo layers are some other slab's)
+        ls::launch_count_layers(ch->g, ch->bb, z0 - lo, z1 - lo, p->iters, k == 0 ? 1 : 0, c->bb.counts, hp->cs, &extra_launches);
+        ok = ck(cudaPeekAtLastError(), "kernel launch") && ck(cudaEventRecord(hp->done[b], hp->cs), "cudaEventRecord") &&
+             ck(cudaStreamWaitEvent(hp->down, hp->done[b], 0), "cudaStreamWaitEvent") &&
+             ck(cudaMemcpyAsync((char*)phi_host + z0 * plane, (const char*)hp->buf[b] + (size_t)(z0 - lo) * plane,
+                                (z1 - z0) * plane, cudaMemcpyDeviceToHost, hp->down), "slab download") &&
+             ck(cudaEventRecord(hp->freed[b], hp->down), "cudaEventRecord");
+    }
+    ck(cudaStreamSynchronize(hp->up), "cudaStreamSynchronize");
+    ck(cudaStreamSynchronize(hp->cs), "cudaStreamSynchronize");
+    ck(cudaStreamSynchronize(hp->down), "cudaStreamSynchronize");
+    c->launches += ch->launches - child_launches0 + extra_launches;
+    c->band_valid = false;      // the windows' bands live in the child ctx; this ctx holds none
+    c->chain_phi = nullptr;
+    if (st != LS_OK) return st;
+    if (ce != cudaSuccess) { cudaGetLastError(); return cuda_fail(ce, what); }
+    return LS_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 const char* ls_status_str(ls_status s) {
@@ -364,6 +527,7 @@ ls_status ls_destroy(ls_ctx* c) {
                    bb.T_masks, bb.N_masks, c->residual, c->scratch, c->dev_phi, c->dev_F, c->snap[0], c->snap[1]};
     for (void* p : dev)
         if (p) cudaFree(p);
+    pipe_destroy(c->pipe);
     if (c->copy_stream) {
         cudaStreamSynchronize(c->copy_stream);
         cudaStreamDestroy(c->copy_stream);
@@ -567,12 +731,14 @@ ls_status ls_step_host(ls_ctx* c, void* phi_host, const void* F_host, const ls_p
     if ((st = ensure_field(c, &c->dev_phi)) != LS_OK) return st;
     if ((st = ensure_field(c, &c->dev_F)) != LS_OK) return st;
     const size_t bytes = (size_t)c->n * c->elem;
-    LS_CK(cudaMemcpyAsync(c->dev_phi, phi_host, bytes, cudaMemcpyHostToDevice, c->stream));
+    const int zs = pipe_slab_layers(c, p, n_steps);
     if (F_host) {
         c->dev_F_valid = false;
         LS_CK(cudaMemcpyAsync(c->dev_F, F_host, bytes, cudaMemcpyHostToDevice, c->stream));
         c->dev_F_valid = true;
     }
+    if (zs > 0) return step_host_sliced(c, phi_host, p, zs);   // one step, large grid: H2D / compute / D2H overlapped by z-slabs
+    LS_CK(cudaMemcpyAsync(c->dev_phi, phi_host, bytes, cudaMemcpyHostToDevice, c->stream));
     if (n_steps > 0) {
         ls_params q = *p;
         q.chained = 0;   // the staging field was just overwritten

@@ -651,6 +651,41 @@ bool launch_export(const Geom& g, BandBuffers& bb, bool with_masks, cudaStream_t
     return true;
 }
 
+// |T| + iters * |N| of the band last built, over the z layers [z0, z1) only, added to `out->updates` (and `add_steps` to
+// out->steps): the z-slab pipeline of ls_step_host runs the step on windows with halo layers and must count each point of
+// the grid once.  One thread per mask word (quad, brick j, lz); integer adds commute.
+__global__ void __launch_bounds__(256) k_count_layers(const uint64_t* __restrict__ tmask, const uint64_t* __restrict__ nmask,
+                                                      Geom g, int z0, int z1, int iters, int add_steps, Counts* out) {
+    __shared__ unsigned long long sh[8];
+    const int64_t nwords = (int64_t)g.nquads * 32;
+    unsigned long long v = 0;
+    for (int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; w < nwords; w += (int64_t)gridDim.x * blockDim.x) {
+        const int quad = (int)(w >> 5), lz = (int)(w & 7);
+        const int z = (quad / (g.NQx * g.NBy)) * 8 + lz;
+        if (z >= z0 && z < z1)
+            v += (unsigned long long)__popcll(tmask[w]) + (unsigned long long)iters * (unsigned long long)__popcll(nmask[w]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long t = 0;
+        for (int i = 0; i < 8; ++i) t += sh[i];
+        if (t) atomicAdd(&out->updates, t);
+        if (blockIdx.x == 0 && add_steps) atomicAdd(&out->steps, (unsigned long long)add_steps);
+    }
+}
+
+void launch_count_layers(const Geom& g, const BandBuffers& bb, int z0, int z1, int iters, int add_steps, Counts* out,
+                         cudaStream_t s, int64_t* launches) {
+    const int64_t nwords = (int64_t)g.nquads * 32;
+    const int64_t want = (nwords + 255) / 256, cap = (int64_t)sm_count() * 8;
+    const int grid = (int)(want < cap ? want : cap);
+    k_count_layers<<<grid, 256, 0, s>>>(bb.tmask[bb.tb], bb.nmask, g, z0, z1, iters, add_steps, out);
+    if (launches) *launches += 1;
+}
+
 template void launch_classify<float>(const float*, const Geom&, float, BandBuffers&, cudaStream_t, int64_t*);
 template void launch_classify<double>(const double*, const Geom&, double, BandBuffers&, cudaStream_t, int64_t*);
 

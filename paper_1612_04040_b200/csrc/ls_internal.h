@@ -104,6 +104,12 @@ void launch_build_lists(const Geom& g, BandBuffers& bb, bool incremental, int it
 // counts into Counts (allocates the export scratch on first use; returns false if that fails).
 bool launch_export(const Geom& g, BandBuffers& bb, bool with_masks, cudaStream_t s, int64_t* launches);
 
+// Adds |T| + iters * |N| of the band last built, restricted to the z layers [z0, z1), to out->updates and add_steps to
+// out->steps (`out` may belong to another ctx: the z-slab pipeline of ls_step_host counts each grid point once).
+// Requires tmask[tb] valid for every quad (a whole-grid classify built the band).
+void launch_count_layers(const Geom& g, const BandBuffers& bb, int z0, int z1, int iters, int add_steps, Counts* out,
+                         cudaStream_t s, int64_t* launches);
+
 // ---- stencil parameters -----------------------------------------------------------------------
 template <typename T>
 struct StencilParams {

@@ -318,6 +318,64 @@ def test_step_host_matches_device():
         assert np.array_equal(host_phi, want2)
 
 
+def _wide_band_field(shape, dtype, seed, dx):
+    """As _random_band_field, by broadcasting (26 M cells): a front that crosses every z-slab cut, plus seeded noise."""
+    nz, ny, nx = shape
+    x = np.arange(nx, dtype=np.float64)[None, None, :]
+    y = np.arange(ny, dtype=np.float64)[None, :, None]
+    z = np.arange(nz, dtype=np.float64)[:, None, None]
+    n = nx * ny * nz
+    phi = dx * (4.0 * np.sin(0.37 * x + 0.2) + 3.0 * np.cos(0.29 * y) + 3.5 * np.sin(0.23 * z + 1.0)
+                + 0.8 * (inputs.uniform01(seed, 0, n).reshape(shape) - 0.5))
+    F = 2.0 * inputs.uniform01(seed + 1, 0, n).reshape(shape) - 1.0
+    return np.ascontiguousarray(phi.astype(dtype)), np.ascontiguousarray(F.astype(dtype))
+
+
+@pytest.mark.parametrize("shape,dtype,iters", [((100, 512, 512), np.float32, 5), ((100, 256, 512), np.float64, 4),
+                                               ((100, 512, 512), np.float32, 0), ((70, 500, 601), np.float32, 3)])
+def test_step_host_z_slab_pipeline(shape, dtype, iters):
+    """ls_step_host on a field of >= 64 MiB, one step per call, runs as a pipeline of z-slabs (windows with iters + 1 halo
+    layers on a child ctx; H2D / compute / D2H on three streams).  Bit-identical to the oracle on the whole grid and to the
+    device-resident ls_step; the work counters count every grid point once; a second call (F reused) continues exactly.
+    Shapes: five slabs of 24 layers with a ragged last one (iters 5, 4), seven of 16 (iters 0), and a grid whose rows are
+    not 16-byte multiples (scalar kernels)."""
+    dx = 1.0 / 32
+    phi, F = _wide_band_field(shape, dtype, 77, dx)
+    p = ls.make_params(dx, 0.4 * dx, 0.5 * dx, 3 * dx, 6 * dx, iters, ls.LS_REBUILD_INCREMENTAL)
+    want1, upd1 = orc.step(phi, F, dx, 0.4 * dx, 0.5 * dx, 3 * dx, 6 * dx, iters, 1)
+    want2, upd2 = orc.step(want1, F, dx, 0.4 * dx, 0.5 * dx, 3 * dx, 6 * dx, iters, 1)
+    host = torch.from_numpy(phi.copy()).pin_memory()
+    hF = torch.from_numpy(F).pin_memory()
+    with Ctx(shape, dtype) as ctx:
+        ls.ls_step_host(ctx, host.data_ptr(), hF.data_ptr(), p, 1)
+        got1 = host.numpy().copy()
+        assert np.array_equal(got1, want1), f"max err {max_err_dx(got1, want1, dx)} dx"
+        assert ls.ls_stats(ctx)[:2] == (upd1, 1)
+        ls.ls_step_host(ctx, host.data_ptr(), None, p, 1)       # F stays on the device
+        assert np.array_equal(host.numpy(), want2)
+        assert ls.ls_stats(ctx)[:2] == (upd1 + upd2, 2)
+        # pageable host memory, and the unsliced multi-step call on the same ctx afterwards
+        pageable = phi.copy()
+        ls.ls_step_host(ctx, pageable, None, p, 1)
+        assert np.array_equal(pageable, want1)
+        ls.ls_step_host(ctx, pageable, None, p, 1)
+        assert np.array_equal(pageable, want2)
+        both = phi.copy()
+        ls.ls_step_host(ctx, both, None, p, 2)                    # two steps in one call: not sliced
+        assert np.array_equal(both, want2)
+        ls.ls_band_counts(ctx)                                    # ... which leaves its band on the ctx
+        pageable[...] = phi
+        ls.ls_step_host(ctx, pageable, None, p, 1)
+        assert np.array_equal(pageable, want1)
+        with pytest.raises(ls.LsError):                           # a sliced call leaves none (ls.h)
+            ls.ls_band_counts(ctx)
+    # and the device-resident path agrees (same library, other driver)
+    with Ctx(shape, dtype) as ctx:
+        d_phi, d_F = to_dev(phi), to_dev(F)
+        ls.ls_step(ctx, d_phi, d_F, p, 1)
+        assert np.array_equal(d_phi.cpu().numpy(), want1)
+
+
 def test_dense_cfg2_steps():
     """cfg 2 at 64^3 and three steps at the full 256^3: ping-pong of full-domain advances."""
     for n, steps in ((64, 10), (256, 3)):
