@@ -376,6 +376,26 @@ def test_step_host_z_slab_pipeline(shape, dtype, iters):
         assert np.array_equal(d_phi.cpu().numpy(), want1)
 
 
+def test_step_host_pipeline_at_bench_size():
+    """cfg 4 at its full 1024^3, the call bench.py's e2e leg times: ls_step_host (43 z-slabs in windows of 36 layers)
+    against the device-resident ls_step on every point of the grid, both steps of two chained host calls, and the work
+    counters; the device path itself is pinned to the oracle at this size by test_full_size_late_step_windowed."""
+    w = inputs.config(4)
+    p = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, ls.LS_REBUILD_INCREMENTAL, 0)
+    host = torch.from_numpy(w.phi).clone().pin_memory()
+    with Ctx(w.shape, w.dtype) as ctx:
+        d_phi, d_F = to_dev(w.phi), to_dev(w.F)
+        ls.ls_step(ctx, d_phi, d_F, p, 1)
+        upd1 = ls.ls_stats(ctx)[0]
+        ls.ls_stats_reset(ctx)
+        ls.ls_step_host(ctx, host.data_ptr(), w.F, p, 1)
+        assert ls.ls_stats(ctx)[:2] == (upd1, 1)
+        assert torch.equal(host.cuda(), d_phi)
+        ls.ls_step(ctx, d_phi, d_F, p, 1)
+        ls.ls_step_host(ctx, host.data_ptr(), None, p, 1)
+        assert torch.equal(host.cuda(), d_phi)
+
+
 def test_dense_cfg2_steps():
     """cfg 2 at 64^3 and three steps at the full 256^3: ping-pong of full-domain advances."""
     for n, steps in ((64, 10), (256, 3)):
