@@ -86,6 +86,8 @@ def parse_args():
     ap.add_argument("--rebuild", default="incremental", choices=["incremental", "full"])
     ap.add_argument("--fuse", type=int, default=0, choices=[0, 1, 2],
                     help="reinit sweeps per launch: 0 = library default (1), 1 = one sweep per launch, 2 = temporal blocking")
+    ap.add_argument("--tile-min-cells", type=int, default=-1,
+                    help="ls_tile_threshold: grids below it take the scalar band kernels (-1 = library default, 0 = tiled wherever possible)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-full-rebuild", action="store_true", help="skip the short LS_REBUILD_FULL run of the same workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -271,6 +273,7 @@ def run_ours(args):
     d_F = h_F.cuda(non_blocking=True) if h_F is not None else None
     stream = torch.cuda.current_stream()
     ctx = ls.ls_create(w.nx, w.ny, w.nz, ls.LS_F32 if esz == 4 else ls.LS_F64, stream.cuda_stream)
+    ls.ls_tile_threshold(ctx, args.tile_min_cells)
     p0 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild, 0, args.fuse)
     p1 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild, 1, args.fuse)
     out = {}
@@ -391,7 +394,7 @@ def report(args, w, out, world, K, W, esz):
             return None
         us = ms / n * 1e3
         ach = alg_bytes / (us * 1e-6) * 1e-9
-        row = ncu.get((wl, key))
+        row = ncu.get((wl, key)) if key else None   # scalar band kernels: one ncu class for Advance and sweeps, no per-kind traffic
         traffic = (float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])) if row else None
         r = {"bound": "hbm", "kernel": what, "achieved": ach, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
              "frac": ach / peak, "traffic": traffic, "traffic_source": ncu_note if row else None,
@@ -411,8 +414,12 @@ def report(args, w, out, world, K, W, esz):
     if w.mode == "band":
         # reinit sweep: read + write of every N point (2w) + the quad's item list (2 B per item ~ 0.6 B per point) and
         # list entry; Advance: phi, F read and phi-bar written on T (3w), halo read on N \ T (w), same lists
-        roofline = roof("reinit", "reinit", "k_band_tile<K=1> (one Step 3 sweep, eq. 12-13)", 2 * esz * nN_pts + 68 * bN)
-        roofline_advance = roof("advance", "advance", "k_band_tile<ADV> (Step 2, eq. 3-8)",
+        # which band kernels ran: the library's rule (ls.h, ls_tile_threshold) restated for the label only
+        thr = 4_000_000 if args.tile_min_cells < 0 else args.tile_min_cells
+        tiled = w.n_points >= thr and (w.nx * esz) % 16 == 0
+        kr, ka = ("k_band_tile<K=1>", "k_band_tile<ADV>") if tiled else ("k_band_scalar<kReinit>", "k_band_scalar<kAdvance>")
+        roofline = roof("reinit", "reinit" if tiled else None, kr + " (one Step 3 sweep, eq. 12-13)", 2 * esz * nN_pts + 68 * bN)
+        roofline_advance = roof("advance", "advance" if tiled else None, ka + " (Step 2, eq. 3-8)",
                                 3 * esz * nT_pts + esz * (nN_pts - nT_pts) + 68 * bN)
     elif w.mode == "dense":
         roofline = roof("advance", "advance_dense", "k_advance_dense2 (full-domain Step 2, c == 1)", 3 * esz * w.n_points)
@@ -436,7 +443,8 @@ def report(args, w, out, world, K, W, esz):
         "dtype": "f32" if esz == 4 else "f64", "data": "synthetic",
         "config": {"workload": workload_name(w), "step": unit_name, "iters": w.iters, "gamma_dx": w.gamma / w.dx,
                    "beta_dx": w.beta / w.dx, "dt_dx": w.dt / w.dx, "dtau_dx": w.dtau / w.dx,
-                   "rebuild": args.rebuild, "fuse": args.fuse or 1, "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "rebuild": args.rebuild, "fuse": args.fuse or 1,
+                   "tile_min_cells": "library default (4 M cells: smaller grids take the scalar band kernels)" if args.tile_min_cells < 0 else args.tile_min_cells, "parallelism": "replicas only" if world > 1 else "1 GPU",
                    "band_last_step": dict(zip(("T_points", "N_points", "T_bricks", "N_bricks"), out["band"])),
                    "updates_per_step": out["updates"] / K,
                    "l2": "inputs larger than L2 (fields >= 0.5 GiB each; one pass touches more than the 126 MB L2)"

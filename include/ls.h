@@ -185,6 +185,14 @@ ls_status ls_step_host(ls_ctx* ctx, void* phi_host, const void* F_host, const ls
 ls_status ls_step_snapshots(ls_ctx* ctx, void* phi, const void* F, const ls_params* p, int32_t n_steps,
                             int32_t every, void* host_out, int32_t* n_written);
 
+/* Which band kernels a ctx uses.  The tiled kernels (32 x 8 x 8 tiles staged in shared memory by producer warps) need
+ * rows that are 16-byte multiples and 16-byte aligned fields; everything else takes the scalar kernels (one CTA per
+ * brick, any shape).  Both give the same bits.  On a grid of fewer than min_cells points the scalar kernels are used
+ * even where the tiled ones could run: a tiled launch needs ~12 us to fill its pipeline, more than a scalar launch takes
+ * on a small band.  Default 4 000 000 (the measured crossover on a B200: 160^3); 0 = tiled wherever possible;
+ * negative = restore the default.  Takes effect from the next band launch. */
+ls_status ls_tile_threshold(ls_ctx* ctx, int64_t min_cells);
+
 /* Work counters since ls_create / the last ls_stats_reset: band point updates
  * sum_steps(|T_s| + iters*|N_s|) (dense advance: nx*ny*nz per call), narrow-band steps done, and
  * kernels launched by this ctx.  HOST out-pointers, any may be NULL.  Synchronises. */

@@ -27,6 +27,7 @@ SYMBOLS = (
     "ls_status_str", "ls_last_cuda_error", "ls_create", "ls_destroy", "ls_build_band", "ls_band_counts",
     "ls_band_export", "ls_advance", "ls_reinit", "ls_reinit_tol", "ls_step", "ls_step_host", "ls_stats",
     "ls_stats_reset", "ls_profile_enable", "ls_profile_read", "ls_profile_reset", "ls_selftest_math", "ls_step_snapshots",
+    "ls_tile_threshold",
 )
 # every symbol include/ls_static.h declares (tests/test_zz_no_alloc.py checks them)
 STATIC_SYMBOLS = ("ls_tube_static_setup", "ls_tube_static", "ls_tube_static_error")
@@ -80,6 +81,7 @@ def lib() -> C.CDLL:
         L.ls_profile_read.argtypes = [_P, _I, C.POINTER(_D), C.POINTER(_L)]
         L.ls_profile_reset.argtypes = [_P]
         L.ls_step_snapshots.argtypes = [_P, _P, _P, C.POINTER(ls_params), _I, _I, _P, C.POINTER(_I)]
+        L.ls_tile_threshold.argtypes = [_P, _L]
         L.ls_selftest_math.argtypes = [_P, C.c_uint64, _L, _D, _D, _D, _D, C.POINTER(_L)]
         for name in SYMBOLS[2:]:
             getattr(L, name).restype = C.c_int
@@ -195,6 +197,11 @@ def ls_stats(ctx: int):
 
 def ls_stats_reset(ctx: int) -> None:
     _ck(lib().ls_stats_reset(_P(ctx)), "ls_stats_reset")
+
+
+def ls_tile_threshold(ctx: int, min_cells: int) -> None:
+    """0 = tiled kernels wherever they can run; negative = the library default (4 000 000 cells)."""
+    _ck(lib().ls_tile_threshold(_P(ctx), min_cells), "ls_tile_threshold")
 
 
 def ls_profile_enable(ctx: int, on: bool) -> None:

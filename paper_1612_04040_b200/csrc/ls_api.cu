@@ -42,6 +42,7 @@ struct ls_ctx {
     double chain_gamma;
     bool chain_have_T;       // tmask[tb ^ 1] holds the T masks of the current phi (emitted by the last sweep)
     bool flip;               // list walking direction of the next band launch
+    int64_t tile_min_cells;  // ls_tile_threshold
     // per-kernel device timing (ls_profile_*)
     bool prof_on;
     struct ProfRec { int kind; cudaEvent_t a, b; };
@@ -144,12 +145,20 @@ bool bad_band_params(double dx, double beta, double gamma) {
     return !(beta > 0 && beta < gamma);
 }
 
+// Default of ls_tile_threshold: grids below it take the scalar band kernels.  A tiled launch costs ~12 us before its
+// first tile is through the pipeline (ticket -> list entry -> item list -> gather -> compute), which is more than the
+// scalar kernel's whole run time on a small band: cfg 1 shapes on a B200, us per step tiled / scalar: 64^3 112 / 65,
+// 96^3 128 / 88, 128^3 133 / 108, 160^3 140 / 138, 200^3 133 / 172, 256^3 135 / 238.
+#ifndef LS_TILE_MIN_CELLS
+#define LS_TILE_MIN_CELLS 4000000
+#endif
+
 // One band launch: the tile kernels where they can address the grid, else the scalar kernels.
 template <typename T>
 void band_launch(ls_ctx* c, const T* src, const T* F, T* dst, const ls::StencilParams<T>& p, ls::BandOp op) {
     op.reverse = c->flip;
     c->flip = !c->flip;
-    if (!op.copy && ls::tile_usable<T>(c->g, src, F, dst) &&
+    if (!op.copy && c->n >= c->tile_min_cells && ls::tile_usable<T>(c->g, src, F, dst) &&
         ls::launch_band_tile<T>(src, F, dst, c->g, p, c->bb, op, c->stream, &c->launches))
         return;
     ls::launch_band_scalar<T>(src, F, dst, c->g, p, c->bb, op, c->stream, &c->launches);
@@ -233,7 +242,7 @@ ls_status step_impl(ls_ctx* c, T* phi, const T* F, const ls_params* p, int n_ste
         // Step 3: `iters` sweeps in launches of 2 (temporal blocking, tile path only) or 1.  The number of
         // launches should be odd so that the last one lands in phi; if it cannot be (iters == 0, or an even
         // count on the scalar path), the band copy below moves the result.
-        const bool can_fuse = p->fuse == 2 && ls::tile_usable<T>(c->g, phi, S, (const void*)nullptr);
+        const bool can_fuse = p->fuse == 2 && c->n >= c->tile_min_cells && ls::tile_usable<T>(c->g, phi, S, (const void*)nullptr);
         int pairs = can_fuse ? p->iters / 2 : 0, singles = p->iters - 2 * pairs;
         if (pairs > 0 && ((pairs + singles) & 1) == 0) { pairs -= 1; singles += 2; }
         for (int l = 0; l < pairs + singles; ++l) {
@@ -386,6 +395,7 @@ ls_status step_host_sliced(ls_ctx* c, void* phi_host, const ls_params* p, int zs
     if (st != LS_OK) return st;
     HostPipe* hp = c->pipe;
     ls_ctx* ch = hp->child;
+    ch->tile_min_cells = c->tile_min_cells <= c->n ? 0 : ch->n + 1;   // the windows take the path the whole grid would
     const int nz = c->g.nz, L = hp->L, K = (nz + zs - 1) / zs;
     const size_t plane = (size_t)c->g.nx * c->g.ny * c->elem;
     ls_params q = *p;
@@ -479,6 +489,7 @@ ls_status ls_create(int32_t nx, int32_t ny, int32_t nz, ls_dtype dtype, void* cu
     c->stream = (cudaStream_t)cuda_stream;
     c->elem = dtype == LS_F32 ? 4 : 8;
     c->n = (int64_t)nx * ny * nz;
+    c->tile_min_cells = LS_TILE_MIN_CELLS;
     c->prof_recs = new (std::nothrow) std::vector<ls_ctx::ProfRec>();
     c->prof_pool = new (std::nothrow) std::vector<cudaEvent_t>();
     if (!c->prof_recs || !c->prof_pool) { delete c->prof_recs; delete c->prof_pool; delete c; return LS_ERR_ALLOC; }
@@ -810,6 +821,12 @@ ls_status ls_stats(ls_ctx* c, int64_t* point_updates, int64_t* steps, int64_t* k
     if (point_updates) *point_updates = (int64_t)c->host_counts->updates + c->dense_updates;
     if (steps) *steps = (int64_t)c->host_counts->steps;
     if (kernel_launches) *kernel_launches = c->launches;
+    return LS_OK;
+}
+
+ls_status ls_tile_threshold(ls_ctx* c, int64_t min_cells) {
+    if (!c) return LS_ERR_ARG;
+    c->tile_min_cells = min_cells < 0 ? (int64_t)LS_TILE_MIN_CELLS : min_cells;
     return LS_OK;
 }
 

@@ -25,11 +25,15 @@ def to_dev(a: np.ndarray) -> torch.Tensor:
 
 
 class Ctx:
-    """ctx bound to torch's current stream."""
+    """ctx bound to torch's current stream.  tile_min_cells = 0 (the default here): the tiled band kernels wherever they
+    can run, so that the small parity shapes exercise them; None: the library's own threshold (small grids take the
+    scalar kernels even when their rows are aligned)."""
 
-    def __init__(self, shape, dtype):
+    def __init__(self, shape, dtype, tile_min_cells=0):
         nz, ny, nx = shape
         self.h = ls.ls_create(nx, ny, nz, dtype_code(dtype), torch.cuda.current_stream().cuda_stream)
+        if tile_min_cells is not None:
+            ls.ls_tile_threshold(self.h, tile_min_cells)
 
     def __enter__(self):
         return self.h

@@ -58,6 +58,7 @@ def test_bad_arguments_rejected_before_cuda(lib):
     assert lib.ls_step(None, None, None, C.byref(p), 1) == ls.LS_ERR_ARG
     assert lib.ls_build_band(None, None, 1.0, 1.0) == ls.LS_ERR_ARG
     assert lib.ls_destroy(None) == ls.LS_OK
+    assert lib.ls_tile_threshold(None, 0) == ls.LS_ERR_ARG
 
 
 def test_no_device_fails_loudly(lib):

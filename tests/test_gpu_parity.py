@@ -396,6 +396,29 @@ def test_step_host_pipeline_at_bench_size():
         assert torch.equal(host.cuda(), d_phi)
 
 
+@pytest.mark.parametrize("n,dtype", [(32, np.float32), (64, np.float32), (64, np.float64), (48, np.float32)])
+def test_library_kernel_choice_on_small_grids(n, dtype):
+    """Ctx() in these tests forces the tiled band kernels so that the small shapes exercise them; the library's own
+    choice (ls_tile_threshold default: scalar kernels below 4 M cells even on aligned rows) must give the same bits,
+    step by step, in both rebuild modes, chained and not; switching the threshold between chained calls is allowed."""
+    w = inputs.config(1, n=n)
+    phi0, F0 = w.phi.astype(dtype), w.F.astype(dtype)
+    want, upd = orc.step(phi0, F0, w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, 6)
+    for rebuild in (ls.LS_REBUILD_INCREMENTAL, ls.LS_REBUILD_FULL):
+        p0 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild, 0)
+        p1 = ls.make_params(w.dx, w.dt, w.dtau, w.beta, w.gamma, w.iters, rebuild, 1)
+        with Ctx(w.shape, dtype, tile_min_cells=None) as ctx:
+            d_phi, d_F = to_dev(phi0), to_dev(F0)
+            ls.ls_step(ctx, d_phi, d_F, p0, 2)
+            ls.ls_step(ctx, d_phi, d_F, p1, 1)
+            ls.ls_tile_threshold(ctx, 0)            # tiled from here on
+            ls.ls_step(ctx, d_phi, d_F, p1, 1)
+            ls.ls_tile_threshold(ctx, -1)           # and back to the default
+            ls.ls_step(ctx, d_phi, d_F, p1, 2)
+            assert np.array_equal(d_phi.cpu().numpy(), want)
+            assert ls.ls_stats(ctx)[:2] == (upd, 6)
+
+
 def test_dense_cfg2_steps():
     """cfg 2 at 64^3 and three steps at the full 256^3: ping-pong of full-domain advances."""
     for n, steps in ((64, 10), (256, 3)):
