@@ -147,8 +147,8 @@ bool bad_band_params(double dx, double beta, double gamma) {
 
 // Default of ls_tile_threshold: grids below it take the scalar band kernels.  A tiled launch costs ~12 us before its
 // first tile is through the pipeline (ticket -> list entry -> item list -> gather -> compute), which is more than the
-// scalar kernel's whole run time on a small band: cfg 1 shapes on a B200, us per step tiled / scalar: 64^3 112 / 65,
-// 96^3 128 / 88, 128^3 133 / 108, 160^3 140 / 138, 200^3 133 / 172, 256^3 135 / 238.
+// scalar kernel's whole run time on a small band: cfg 1 shapes on a B200, us per step tiled / scalar: 64^3 104 / 56,
+// 96^3 109 / 69, 128^3 114 / 88, 160^3 118 / 117, 200^3 116 / 157, 256^3 119 / 223.
 #ifndef LS_TILE_MIN_CELLS
 #define LS_TILE_MIN_CELLS 4000000
 #endif

@@ -179,16 +179,19 @@ __global__ void __launch_bounds__(kDilateWarps * 32) k_dilate_items(Geom g, Dila
     // bytes are loaded unconditionally (no dependent branch between them): what this kernel waits for is the flags.
     const uint8_t* gate = a.tgate != nullptr ? a.tgate : a.qflagT;
     auto tvalid = [&](bool inside, int q) -> unsigned { return inside ? ((a.qflagT[q] != 0) & (gate[q] != 0) ? 1u : 0u) : 0u; };
-    // A warp turn takes 32 consecutive candidates: each lane resolves one (which quad, does another candidate own
+    // A warp turn takes up to 32 consecutive candidates: each lane resolves one (which quad, does another candidate own
     // it, which of the quad and its six face neighbours hold valid T masks) with its flag loads in flight together;
     // the quads that can hold an N point are then processed one after the other by the whole warp.
-    for (int64_t w0 = ((int64_t)blockIdx.x * kDilateWarps + wib) * 32; w0 < ncand; w0 += nwarps * 32) {
+    // On a short candidate list a turn takes fewer than 32 (`per`), so that the quads to process — a serial loop per
+    // warp — spread over all warps of the grid instead of piling up on the first ncand / 32 of them.
+    const int per = (int)(ncand >= nwarps * 32 ? 32 : (ncand + nwarps - 1) / nwarps < 1 ? 1 : (ncand + nwarps - 1) / nwarps);
+    for (int64_t w0 = ((int64_t)blockIdx.x * kDilateWarps + wib) * per; w0 < ncand; w0 += nwarps * per) {
     int mine = -1, my_x = 0, my_y = 0, my_z = 0;
     unsigned my_valid = 0;   // bit 0: the quad itself, bits 1..6: its -x, +x, -y, +y, -z, +z neighbour
     {
         const int64_t wid = w0 + lane;
         int c = -1;
-        if (wid < ncand) c = INCREMENTAL ? candidate_quad(g, a, wid, nprev, nstale) : (int)wid;
+        if (lane < per && wid < ncand) c = INCREMENTAL ? candidate_quad(g, a, wid, nprev, nstale) : (int)wid;
         if (c >= 0) {
             const int cx = c % g.NQx, cy = (c / g.NQx) % g.NBy, cz = c / szq;
             my_x = cx; my_y = cy; my_z = cz;
@@ -432,14 +435,16 @@ __global__ void __launch_bounds__(kCompactThreads) k_compact(const uint8_t* __re
         mine += __popc(flag_bits16(qflagN, t * kCompactTile + (int64_t)threadIdx.x * kFlagsPerThread, nquads));
     int total;
     cta_exclusive_scan(mine, s_warp, &total);
-    if (threadIdx.x == 0) {
-        partials[blockIdx.x] = total;
-        __threadfence();
-        atomicAdd(&counts->bar, 1ull);
-        while (*reinterpret_cast<volatile unsigned long long*>(&counts->bar) < bar_target) {}
-        __threadfence();
+    if (G > 1) {   // a single CTA (small grids) has nobody to wait for
+        if (threadIdx.x == 0) {
+            partials[blockIdx.x] = total;
+            __threadfence();
+            atomicAdd(&counts->bar, 1ull);
+            while (*reinterpret_cast<volatile unsigned long long*>(&counts->bar) < bar_target) {}
+            __threadfence();
+        }
+        __syncthreads();
     }
-    __syncthreads();
     // phase 2: my base = sum of the partials before me
     int base = 0;
     {
