@@ -364,6 +364,11 @@ def test_step_host_z_slab_pipeline(shape, dtype, iters):
         ls.ls_step_host(ctx, both, None, p, 2)                    # two steps in one call: not sliced
         assert np.array_equal(both, want2)
         ls.ls_band_counts(ctx)                                    # ... which leaves its band on the ctx
+        if iters == 5:   # the windows honour the other step options too: paper-style full rebuild, two fused sweeps per launch
+            p_alt = ls.make_params(dx, 0.4 * dx, 0.5 * dx, 3 * dx, 6 * dx, iters, ls.LS_REBUILD_FULL, 0, 2)
+            pageable[...] = phi
+            ls.ls_step_host(ctx, pageable, None, p_alt, 1)
+            assert np.array_equal(pageable, want1)
         pageable[...] = phi
         ls.ls_step_host(ctx, pageable, None, p, 1)
         assert np.array_equal(pageable, want1)
