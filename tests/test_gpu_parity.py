@@ -332,13 +332,14 @@ def _wide_band_field(shape, dtype, seed, dx):
 
 
 @pytest.mark.parametrize("shape,dtype,iters", [((100, 512, 512), np.float32, 5), ((100, 256, 512), np.float64, 4),
-                                               ((100, 512, 512), np.float32, 0), ((70, 500, 601), np.float32, 3)])
+                                               ((100, 512, 512), np.float32, 0), ((70, 500, 601), np.float32, 3),
+                                               ((90, 384, 512), np.float32, 1), ((90, 384, 512), np.float32, 2)])
 def test_step_host_z_slab_pipeline(shape, dtype, iters):
     """ls_step_host on a field of >= 64 MiB, one step per call, runs as a pipeline of z-slabs (windows with iters + 1 halo
     layers on a child ctx; H2D / compute / D2H on three streams).  Bit-identical to the oracle on the whole grid and to the
     device-resident ls_step; the work counters count every grid point once; a second call (F reused) continues exactly.
-    Shapes: five slabs of 24 layers with a ragged last one (iters 5, 4), seven of 16 (iters 0), and a grid whose rows are
-    not 16-byte multiples (scalar kernels)."""
+    Shapes: five slabs of 24 layers with a ragged last one (iters 5, 4), seven of 16 (iters 0), a grid whose rows are
+    not 16-byte multiples (scalar kernels), and 22-layer slabs with halos of 2 and 3 layers (iters 1, 2)."""
     dx = 1.0 / 32
     phi, F = _wide_band_field(shape, dtype, 77, dx)
     p = ls.make_params(dx, 0.4 * dx, 0.5 * dx, 3 * dx, 6 * dx, iters, ls.LS_REBUILD_INCREMENTAL)
